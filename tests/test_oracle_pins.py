@@ -1,0 +1,585 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these compares the oracle with itself through the same routine: they use closed forms,
+conservation laws, identities printed in the paper (Eq 7, Eq 8, Eq 10), reductions between
+models that are implemented along different routes, hand-stepped tiny lattices and analytic
+solutions (shear-wave decay, Poiseuille profile).  CPU only.
+"""
+import itertools
+
+import numpy as np
+import pytest
+
+from paper_2010_11751_b200 import inputs
+
+ALL_MODELS = ["BGK_W2", "BGK_NW4", "TRT", "RM", "HM", "CM", "CHM", "K", "RR", "REG"]
+W2_MODELS = ("BGK_W2", "TRT", "REG")
+LATTICES = (19, 27)
+
+
+def eq_kind(model):
+    return "w2" if model in W2_MODELS else "ext"
+
+
+def perturbed(o, Q, model, rng, amp=1e-3, rho=1.03, u=(0.04, -0.03, 0.05)):
+    E = o.equilibrium(Q, eq_kind(model), rho, u)
+    return E + amp * rng.uniform(-1, 1, Q) * E
+
+
+# ------------------------------------------------------------------ lattice tables (R7, R8)
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_lattice_tables(oracle, Q):
+    c, t, opp, mom = oracle.lattice(Q)
+    # c_0 = (-1,0,0) = -c_10 in D3Q19
+    assert tuple(c[0]) == (-1, 0, 0)
+    if Q == 19:
+        assert tuple(c[10]) == (1, 0, 0) and opp[0] == 10
+    assert len({tuple(v) for v in c}) == Q
+    assert np.all(c[opp] == -c) and np.all(opp[opp] == np.arange(Q))
+    assert abs(t.sum() - 1.0) < 1e-15
+    assert np.allclose(np.einsum("k,ka->a", t, c), 0.0, atol=1e-16)
+    assert np.allclose(np.einsum("k,ka,kb->ab", t, c, c), np.eye(3) / 3.0, atol=1e-15)
+    # fourth-order isotropy: sum t c_a c_b c_c c_d = (1/9)(d_ab d_cd + d_ac d_bd + d_ad d_bc)
+    d = np.eye(3)
+    iso = (np.einsum("ab,cd->abcd", d, d) + np.einsum("ac,bd->abcd", d, d) + np.einsum("ad,bc->abcd", d, d)) / 9.0
+    assert np.allclose(np.einsum("k,ka,kb,kc,kd->abcd", t, c, c, c, c), iso, atol=1e-15)
+    # moment set: lower set of size Q
+    ms = {tuple(m) for m in mom}
+    assert len(ms) == Q
+    for p, q, r in ms:
+        for a, b, cc in itertools.product(range(p + 1), range(q + 1), range(r + 1)):
+            assert (a, b, cc) in ms
+
+
+# ------------------------------------------------------------------ equilibria
+
+@pytest.mark.parametrize("Q", LATTICES)
+@pytest.mark.parametrize("kind", ["w2", "ext"])
+def test_equilibrium_moments(oracle, Q, kind):
+    """Mass, momentum and the second moment rho(uu + I/3) of both equilibria (R1 pins the 1.5)."""
+    c, t, opp, mom = oracle.lattice(Q)
+    rho, u = 1.07, np.array([0.05, -0.02, 0.08])
+    E = oracle.equilibrium(Q, kind, rho, u)
+    assert abs(E.sum() - rho) < 1e-15
+    assert np.allclose(c.T @ E, rho * u, atol=1e-16)
+    P = np.einsum("k,ka,kb->ab", E, c, c)
+    assert np.allclose(P, rho * (np.outer(u, u) + np.eye(3) / 3.0), atol=1e-15)
+
+
+def test_w2_equilibrium_rest_state(oracle):
+    """At u = 0 Eq 6 must return rho t_k, with the textbook weights typed here."""
+    for Q, weights in ((19, {0: 1 / 3, 1: 1 / 18, 2: 1 / 36}), (27, {0: 8 / 27, 1: 2 / 27, 2: 1 / 54, 3: 1 / 216})):
+        c, *_ = oracle.lattice(Q)
+        E = oracle.equilibrium(Q, "w2", 2.0, [0, 0, 0])
+        expect = np.array([2.0 * weights[int((v * v).sum())] for v in c])
+        assert np.abs(E - expect).max() < 1e-16
+
+
+def test_ext_equilibrium_d3q27_product_form(oracle):
+    """On D3Q27 the extended equilibrium is rho prod_a phi_{c_a}(u_a), phi_0 = 2/3 - v^2, phi_+- = (v^2 + 1/3 +- v)/2."""
+    c, *_ = oracle.lattice(27)
+    rho, u = 0.93, np.array([0.07, 0.02, -0.05])
+    phi = lambda ci, v: (2 / 3 - v * v) if ci == 0 else 0.5 * (v * v + 1 / 3 + ci * v)
+    expect = np.array([rho * phi(v[0], u[0]) * phi(v[1], u[1]) * phi(v[2], u[2]) for v in c])
+    assert np.abs(oracle.equilibrium(27, "ext", rho, u) - expect).max() < 1e-15
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_eq7_opposite_pair_identity(oracle, Q):
+    """PAPER.md Eq 7 (L315): E_kbar = E_k - 6 rho t_k c_k.u."""
+    c, t, opp, _ = oracle.lattice(Q)
+    rho, u = 1.02, np.array([0.03, 0.06, -0.04])
+    E = oracle.equilibrium(Q, "w2", rho, u)
+    assert np.abs(E[opp] - (E - 6 * rho * t * (c @ u))).max() < 1e-16
+
+
+def test_eq8_eq10_raw_moment_inverse_d3q19(oracle):
+    """PAPER.md Eq 8-10 (L321-327) with M* = M (R16: Eq 12 defines rho M) must return f_0 and f_10."""
+    rng = np.random.default_rng(1)
+    c, t, opp, mom = oracle.lattice(19)
+    f = rng.uniform(0.01, 0.2, 19)
+    M = oracle.moments(19, "raw", f)
+    idx = {tuple(m): i for i, m in enumerate(mom)}
+    g = lambda p, q, r: M[idx[(p, q, r)]]
+    f0 = 0.5 * (-g(1, 0, 0) + g(2, 0, 0) + g(1, 2, 0) + g(1, 0, 2) - g(2, 2, 0) - g(2, 0, 2))
+    f10 = 0.5 * (g(1, 0, 0) + g(2, 0, 0) - g(1, 2, 0) - g(1, 0, 2) - g(2, 2, 0) - g(2, 0, 2))   # R2 reading of Eq 9
+    assert abs(f0 - f[0]) < 1e-16 and abs(f10 - f[10]) < 1e-16
+    assert abs(f0 - (f10 - (g(1, 0, 0) - g(1, 2, 0) - g(1, 0, 2)))) < 1e-16      # Eq 10
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_raw_moments_are_eq12(oracle, Q):
+    rng = np.random.default_rng(2)
+    c, t, opp, mom = oracle.lattice(Q)
+    f = rng.uniform(0.01, 0.2, Q)
+    M = oracle.moments(Q, "raw", f)
+    expect = np.array([(c[:, 0] ** p * c[:, 1] ** q * c[:, 2] ** r * f).sum() for p, q, r in mom])
+    assert np.abs(M - expect).max() < 1e-15
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_equilibrium_moments_closed_forms(oracle, Q):
+    """HM of f^eq,x -> rho u^p u^q u^r; CM -> rho {1,0,1/3} products; CHM -> 0 beyond order 0."""
+    c, t, opp, mom = oracle.lattice(Q)
+    rho, u = 1.05, np.array([0.06, -0.03, 0.02])
+    E = oracle.equilibrium(Q, "ext", rho, u)
+    hm = oracle.moments(Q, "hermite", E)
+    cm = oracle.moments(Q, "central", E, u)
+    chm = oracle.moments(Q, "central_hermite", E, u)
+    cm1 = [1.0, 0.0, 1 / 3]
+    for i, (p, q, r) in enumerate(mom):
+        assert abs(hm[i] - rho * u[0] ** p * u[1] ** q * u[2] ** r) < 1e-15
+        assert abs(cm[i] - rho * cm1[p] * cm1[q] * cm1[r]) < 1e-15
+        assert abs(chm[i] - (rho if p + q + r == 0 else 0.0)) < 1e-15
+
+
+# ------------------------------------------------------------------ P1, P12: fixed point, conservation
+
+@pytest.mark.parametrize("Q", LATTICES)
+@pytest.mark.parametrize("model", ALL_MODELS)
+def test_p1_equilibrium_is_fixed_point(oracle, Q, model):
+    rng = np.random.default_rng(3)
+    for _ in range(5):
+        rho = rng.uniform(0.9, 1.1)
+        u = rng.uniform(-0.1, 0.1, 3) / np.sqrt(3)
+        E = oracle.equilibrium(Q, eq_kind(model), rho, u)
+        for omega in (0.6, 1.0, 1.93):
+            assert np.abs(oracle.collide(Q, model, E, omega) - E).max() < 1e-15
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+@pytest.mark.parametrize("model", ALL_MODELS)
+def test_p12_collision_conserves_mass_momentum(oracle, Q, model):
+    rng = np.random.default_rng(4)
+    c, *_ = oracle.lattice(Q)
+    f = perturbed(oracle, Q, model, rng, amp=2e-2)
+    for kw in (dict(), dict(omega_bulk=1.0, omega3=1.3, omega_hi=0.8)):
+        out = oracle.collide(Q, model, f, 1.8, **kw)
+        assert abs(out.sum() - f.sum()) < 1e-15
+        assert np.abs(c.T @ out - c.T @ f).max() < 1e-15
+
+
+# ------------------------------------------------------------------ P7, P8, P9, P13, P14, P15
+
+@pytest.mark.parametrize("Q", LATTICES)
+@pytest.mark.parametrize("model", ["RM", "HM", "CM", "CHM"])
+def test_p7_equal_rates_collapse_to_bgk_nw4(oracle, Q, model):
+    rng = np.random.default_rng(5)
+    f = perturbed(oracle, Q, model, rng)
+    w = 1.7
+    ref = oracle.collide(Q, "BGK_NW4", f, w)
+    out = oracle.collide(Q, model, f, w, omega_bulk=w, omega3=w, omega_hi=w)
+    assert np.abs(out - ref).max() < 2e-15
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_p8_trt_equal_rates_is_bgk(oracle, Q):
+    rng = np.random.default_rng(6)
+    f = perturbed(oracle, Q, "TRT", rng)
+    w = 1.6
+    lam = (1 / w - 0.5) ** 2
+    assert np.abs(oracle.collide(Q, "TRT", f, w, trt_magic=lam) - oracle.collide(Q, "BGK_W2", f, w)).max() < 1e-16
+    # and with Lambda = 1/4 it is a different operator
+    assert np.abs(oracle.collide(Q, "TRT", f, w) - oracle.collide(Q, "BGK_W2", f, w)).max() > 1e-7
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_trt_antisymmetric_rate(oracle, Q):
+    """TRT: the symmetric part relaxes with omega+, the antisymmetric part with omega- = 1/(Lambda/(1/w+ - 1/2) + 1/2)."""
+    rng = np.random.default_rng(7)
+    c, t, opp, _ = oracle.lattice(Q)
+    f = perturbed(oracle, Q, "TRT", rng, amp=1e-2)
+    w, lam = 1.5, 0.25
+    wm = 1.0 / (lam / (1.0 / w - 0.5) + 0.5)
+    out = oracle.collide(Q, "TRT", f, w)
+    E = oracle.equilibrium(Q, "w2", f.sum(), (c.T @ f) / f.sum())
+    sym = lambda g: 0.5 * (g + g[opp])
+    asym = lambda g: 0.5 * (g - g[opp])
+    assert np.abs(sym(out) - E_sym_relax(sym(f), sym(E), w)).max() < 1e-16
+    assert np.abs(asym(out) - E_sym_relax(asym(f), asym(E), wm)).max() < 1e-16
+
+
+def E_sym_relax(g, ge, w):
+    return g - w * (g - ge)
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_p9_regularized_stress(oracle, Q):
+    rng = np.random.default_rng(8)
+    c, t, opp, _ = oracle.lattice(Q)
+    f = perturbed(oracle, Q, "REG", rng, amp=2e-2)
+    w = 1.4
+    out = oracle.collide(Q, "REG", f, w)
+    rho = f.sum()
+    u = (c.T @ f) / rho
+    E = oracle.equilibrium(Q, "w2", rho, u)
+    pi = lambda g: np.einsum("k,ka,kb->ab", g - E, c, c)
+    assert np.abs(pi(out) - (1 - w) * pi(f)).max() < 1e-15
+    assert abs(out.sum() - rho) < 1e-15 and np.abs(c.T @ out - rho * u).max() < 1e-15
+    # the regularised state has no non-hydrodynamic content: applying REG with omega = 0 twice is idempotent
+    once = oracle.collide(Q, "REG", f, 0.0)
+    assert np.abs(oracle.collide(Q, "REG", once, 0.0) - once).max() < 1e-15
+
+
+def test_cumulant_relation_explicit_k220_and_independence(oracle):
+    """The generic moment->cumulant relation against (a) the explicit fourth-order formula for centred
+    variables and (b) a product measure, whose mixed cumulants vanish and whose marginal cumulants
+    are k1 = m1, k2 = m2 - m1^2."""
+    rng = np.random.default_rng(9)
+    for Q in LATTICES:
+        c, t, opp, mom = oracle.lattice(Q)
+        idx = {tuple(m): i for i, m in enumerate(mom)}
+        # (a) centred: first-order moments zero
+        kap = rng.uniform(-0.2, 0.4, Q)
+        kap[idx[(0, 0, 0)]] = 1.0
+        for e in ((1, 0, 0), (0, 1, 0), (0, 0, 1)):
+            kap[idx[e]] = 0.0
+        K = oracle.cumulants_from_moments(Q, kap)
+        g = lambda *m: kap[idx[m]]
+        assert abs(K[idx[(2, 2, 0)]] - (g(2, 2, 0) - g(2, 0, 0) * g(0, 2, 0) - 2 * g(1, 1, 0) ** 2)) < 1e-15
+        assert abs(K[idx[(2, 0, 2)]] - (g(2, 0, 2) - g(2, 0, 0) * g(0, 0, 2) - 2 * g(1, 0, 1) ** 2)) < 1e-15
+        for m in mom:
+            if sum(m) in (2, 3):
+                assert abs(K[idx[tuple(m)]] - g(*m)) < 1e-16
+        if Q == 27:
+            assert abs(K[idx[(2, 1, 1)]] - (g(2, 1, 1) - g(2, 0, 0) * g(0, 1, 1) - 2 * g(1, 1, 0) * g(1, 0, 1))) < 1e-15
+        # round trip
+        back = oracle.moments_from_cumulants(Q, K)
+        assert np.abs(back - kap).max() < 1e-15
+    # (b) product measure on D3Q27
+    c, t, opp, mom = oracle.lattice(27)
+    a = [np.array([1.0, rng.uniform(-0.3, 0.3), rng.uniform(0.3, 0.6)]) for _ in range(3)]
+    kap = np.array([a[0][p] * a[1][q] * a[2][r] for p, q, r in mom])
+    K = oracle.cumulants_from_moments(27, kap)
+    for i, (p, q, r) in enumerate(mom):
+        nz = int(p > 0) + int(q > 0) + int(r > 0)
+        if nz >= 2:
+            assert abs(K[i]) < 1e-15
+        elif nz == 1:
+            ax = 0 if p else 1 if q else 2
+            order = p + q + r
+            expect = a[ax][1] if order == 1 else a[ax][2] - a[ax][1] ** 2
+            assert abs(K[i] - expect) < 1e-15
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_p13_cumulant_fourth_order_equilibrated(oracle, Q):
+    """K with fourth-order rate 1: kappa*_220 = kappa*_200 kappa*_020 + 2 kappa*_110^2 (K*_220 = 0)."""
+    rng = np.random.default_rng(10)
+    c, t, opp, mom = oracle.lattice(Q)
+    idx = {tuple(m): i for i, m in enumerate(mom)}
+    f = perturbed(oracle, Q, "K", rng, amp=2e-2)
+    out = oracle.collide(Q, "K", f, 1.7)
+    rho = out.sum()
+    u = (c.T @ out) / rho
+    kap = oracle.moments(Q, "central", out, u) / rho
+    g = lambda *m: kap[idx[m]]
+    assert abs(g(2, 2, 0) - (g(2, 0, 0) * g(0, 2, 0) + 2 * g(1, 1, 0) ** 2)) < 1e-15
+    assert abs(g(0, 2, 2) - (g(0, 2, 0) * g(0, 0, 2) + 2 * g(0, 1, 1) ** 2)) < 1e-15
+    # third order equilibrated too (rate 1, K = kappa at order 3)
+    assert abs(g(2, 1, 0)) < 1e-15 and abs(g(0, 1, 2)) < 1e-15
+    # second-order off-diagonal relaxes with omega
+    kin = oracle.moments(Q, "central", f, (c.T @ f) / f.sum()) / f.sum()
+    assert abs(g(1, 1, 0) - (1 - 1.7) * kin[idx[(1, 1, 0)]]) < 1e-15
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_p14_default_rates_models_differ(oracle, Q):
+    rng = np.random.default_rng(11)
+    # K differs from CM/CHM only through products of second-order deviations, hence the larger amplitude
+    f = perturbed(oracle, Q, "RM", rng, amp=5e-2)
+    outs = {m: oracle.collide(Q, m, f, 1.8) for m in ("BGK_NW4", "RM", "HM", "CM", "CHM", "K")}
+    names = list(outs)
+    for a, b in itertools.combinations(names, 2):
+        assert np.abs(outs[a] - outs[b]).max() > 1e-7, (a, b)
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_p15_rr_equals_chm_and_hm_limits(oracle, Q):
+    rng = np.random.default_rng(12)
+    f = perturbed(oracle, Q, "RR", rng, amp=1e-2)
+    w = 1.75
+    rr = oracle.collide(Q, "RR", f, w)                                       # default: high orders at rate omega
+    chm = oracle.collide(Q, "CHM", f, w, omega3=1.0, omega_hi=1.0)
+    assert np.abs(rr - chm).max() < 1e-15
+    rr1 = oracle.collide(Q, "RR", f, w, omega3=1.0, omega_hi=1.0)
+    hm = oracle.collide(Q, "HM", f, w, omega3=1.0, omega_hi=1.0)
+    assert np.abs(rr1 - hm).max() < 1e-15
+    assert np.abs(rr - rr1).max() > 1e-8
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_bulk_rate_eq13_15(oracle, Q):
+    """Eq 13-15: trace of the second-order non-equilibrium relaxes with omega_bulk, the deviator with omega;
+    with omega_bulk = omega the three equations reduce to Eq 11 (R3)."""
+    rng = np.random.default_rng(13)
+    c, *_ = oracle.lattice(Q)
+    w, wb = 1.8, 1.0
+    for model in ("RM", "HM", "CM", "CHM", "K", "RR"):
+        f = perturbed(oracle, Q, model, rng, amp=1e-2)
+        rho = f.sum()
+        u = (c.T @ f) / rho
+        E = oracle.equilibrium(Q, "ext", rho, u)
+        pin = np.einsum("k,ka,kb->ab", f - E, c, c)
+        out = oracle.collide(Q, model, f, w, omega_bulk=wb)
+        pout = np.einsum("k,ka,kb->ab", out - E, c, c)
+        tr_in, tr_out = np.trace(pin), np.trace(pout)
+        assert abs(tr_out - (1 - wb) * tr_in) < 2e-15, model
+        dev_in = pin - np.eye(3) * tr_in / 3
+        dev_out = pout - np.eye(3) * tr_out / 3
+        assert np.abs(dev_out - (1 - w) * dev_in).max() < 2e-15, model
+
+
+# ------------------------------------------------------------------ P5: hand-stepped tiny lattices
+
+@pytest.mark.parametrize("Q", LATTICES)
+@pytest.mark.parametrize("model", ["BGK_W2", "CM", "K"])
+def test_p5_single_cell_periodic(oracle, Q, model):
+    """1x1x1 periodic box: streaming is the identity, f(t+1) = Omega(f)."""
+    rng = np.random.default_rng(14)
+    f = perturbed(oracle, Q, model, rng, amp=1e-2)
+    o = oracle.Oracle(1, 1, 1, Q, model, 1.6)
+    o.set_flags(np.zeros(1, dtype=np.uint8))
+    o.set_populations(f.reshape(Q, 1))
+    o.step(1)
+    assert np.array_equal(o.get_populations()[:, 0], oracle.collide(Q, model, f, 1.6))
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_p5_enclosed_cell_bounces_every_link(oracle, Q):
+    """3x3x3 box, only the centre fluid: f_kbar(t+1) = f_out_k - 6 t_k c_k.u_w (Eq 3), per wall type."""
+    rng = np.random.default_rng(15)
+    c, t, opp, _ = oracle.lattice(Q)
+    fl = np.full((3, 3, 3), inputs.WALL, dtype=np.uint8)
+    fl[:, :, 2] = inputs.MOVING
+    fl[1, 1, 1] = inputs.FLUID
+    uw = np.array([0.05, -0.02, 0.01])
+    f = perturbed(oracle, Q, "BGK_W2", rng, amp=1e-2)
+    o = oracle.Oracle(3, 3, 3, Q, "BGK_W2", 1.3)
+    o.set_flags(fl, uw)
+    pops = np.zeros((Q, 27))
+    centre = (1 * 3 + 1) * 3 + 1
+    pops[:, centre] = f
+    o.set_populations(pops)
+    o.step(1)
+    got = o.get_populations()
+    fout = oracle.collide(Q, "BGK_W2", f, 1.3)
+    expect = np.zeros(Q)
+    for k in range(Q):
+        if not c[k].any():
+            expect[k] = fout[k]
+            continue
+        moving = (1 + c[k][2]) == 2          # neighbour lies in the plane iz = 2
+        expect[opp[k]] = fout[k] - (6 * t[k] * (c[k] @ uw) if moving else 0.0)
+    assert np.abs(got[:, centre] - expect).max() < 1e-17
+    mask = np.ones(27, dtype=bool)
+    mask[centre] = False
+    assert np.all(got[:, mask] == 0.0)
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_p5_two_cell_periodic_exchange(oracle, Q):
+    """2x1x1 periodic: populations with c_x != 0 move to the other cell, the rest stay."""
+    rng = np.random.default_rng(16)
+    c, *_ = oracle.lattice(Q)
+    fa = perturbed(oracle, Q, "BGK_W2", rng, amp=1e-2)
+    fb = perturbed(oracle, Q, "BGK_W2", rng, amp=1e-2, rho=0.98, u=(-0.02, 0.01, 0.03))
+    o = oracle.Oracle(2, 1, 1, Q, "BGK_W2", 1.1)
+    o.set_flags(np.zeros(2, dtype=np.uint8))
+    o.set_populations(np.stack([fa, fb], axis=1))
+    o.step(1)
+    got = o.get_populations()
+    oa, ob = oracle.collide(Q, "BGK_W2", fa, 1.1), oracle.collide(Q, "BGK_W2", fb, 1.1)
+    for k in range(Q):
+        if c[k][0] != 0:
+            assert got[k, 0] == ob[k] and got[k, 1] == oa[k]
+        else:
+            assert got[k, 0] == oa[k] and got[k, 1] == ob[k]
+
+
+def test_streaming_moves_each_population_along_its_velocity(oracle):
+    """omega = 0 (no collision for BGK): a single marked population must appear at x + c_k, periodic wrap included."""
+    nx, ny, nz = 4, 3, 5
+    for Q in LATTICES:
+        c, *_ = oracle.lattice(Q)
+        N = nx * ny * nz
+        o = oracle.Oracle(nx, ny, nz, Q, "BGK_W2", 0.0)
+        o.set_flags(np.zeros(N, dtype=np.uint8))
+        pops = np.zeros((Q, N))
+        src = (3, 0, 4)
+        i0 = (src[0] * ny + src[1]) * nz + src[2]
+        pops[:, i0] = 1.0 + np.arange(Q)
+        # a positive background keeps rho > 0 everywhere
+        pops += 1.0
+        o.set_populations(pops)
+        o.step(1)
+        got = o.get_populations()
+        for k in range(Q):
+            dst = ((src[0] + c[k][0]) % nx, (src[1] + c[k][1]) % ny, (src[2] + c[k][2]) % nz)
+            i1 = (dst[0] * ny + dst[1]) * nz + dst[2]
+            assert got[k, i1] == 2.0 + k
+        assert abs(got.sum() - pops.sum()) < 1e-10
+
+
+# ------------------------------------------------------------------ P2, P11: global conservation, symmetry
+
+@pytest.mark.parametrize("Q,model", [(19, "BGK_W2"), (19, "TRT"), (27, "CM"), (27, "K"), (19, "RR"), (27, "REG")])
+def test_p2_periodic_conservation(oracle, Q, model):
+    nx, ny, nz = 6, 5, 7
+    c, *_ = oracle.lattice(Q)
+    rho, u = inputs.seeded_init(nx, ny, nz, seed=3)
+    o = oracle.Oracle(nx, ny, nz, Q, model, 1.7)
+    o.set_flags(inputs.periodic_flags(nx, ny, nz))
+    o.init_equilibrium(rho, u)
+    f0 = o.get_populations()
+    steps = 20
+    o.step(steps)
+    f1 = o.get_populations()
+    m0, m1 = f0.sum(), f1.sum()
+    assert abs(m1 - m0) / m0 < 1e-13 * steps
+    p0, p1 = c.T @ f0.sum(axis=1), c.T @ f1.sum(axis=1)
+    assert np.abs(p1 - p0).max() < 1e-13 * steps * m0 * 0.01
+    assert np.isfinite(f1).all()
+
+
+def test_p2_cavity_mass_conservation_and_p11_mirror_symmetry(oracle):
+    """Cavity from rest: mass conserved to round-off (whole lid plane MOVING, R9) and the field is
+    symmetric under y -> ny-1-y because the lid moves along x."""
+    n = 10
+    c, t, opp, _ = oracle.lattice(19)
+    fl = inputs.cavity_flags(n, n, n)
+    o = oracle.Oracle(n, n, n, 19, "BGK_W2", 1.5)
+    o.set_flags(fl, (inputs.U_LID, 0.0, 0.0))
+    o.init_equilibrium(np.ones(n ** 3), np.zeros((3, n ** 3)))
+    m0 = o.get_populations().sum()
+    o.step(30)
+    f = o.get_populations()
+    assert abs(f.sum() - m0) / m0 < 1e-13
+    rho, u = o.macroscopic()
+    rho = rho.reshape(n, n, n)
+    u = u.reshape(3, n, n, n)
+    assert np.abs(u[0]).max() > 1e-4                      # the lid drives a flow
+    assert np.abs(rho - rho[:, ::-1, :]).max() < 1e-14
+    assert np.abs(u[0] - u[0][:, ::-1, :]).max() < 1e-14
+    assert np.abs(u[1] + u[1][:, ::-1, :]).max() < 1e-14
+    assert np.abs(u[2] - u[2][:, ::-1, :]).max() < 1e-14
+    # the mirror image of direction k is the direction with c_y flipped
+    mirror = np.array([[j for j in range(19) if tuple(c[j]) == (c[k][0], -c[k][1], c[k][2])][0] for k in range(19)])
+    f4 = f.reshape(19, n, n, n)
+    assert np.abs(f4 - f4[mirror][:, :, ::-1, :]).max() < 1e-14
+    # non-fluid cells export zeros
+    assert np.all(f4[:, fl != inputs.FLUID] == 0.0)
+
+
+def test_lid_momentum_injection_first_step(oracle):
+    """From rest, after one step the only momentum in the cavity is what Eq 3 injects on the links
+    that hit the MOVING plane: sum over those links of 6 t_k (c_k.u_w) c_kbar ... closed form."""
+    n = 8
+    c, t, opp, _ = oracle.lattice(19)
+    fl = inputs.cavity_flags(n, n, n)
+    uw = np.array([inputs.U_LID, 0.0, 0.0])
+    o = oracle.Oracle(n, n, n, 19, "BGK_W2", 1.2)
+    o.set_flags(fl, uw)
+    o.init_equilibrium(np.ones(n ** 3), np.zeros((3, n ** 3)))
+    o.step(1)
+    f = o.get_populations()
+    mom = c.T @ f.sum(axis=1)
+    # fluid cells in the layer iz = n-2: (n-2)^2 of them; links with c_z = +1 hit the lid
+    nlayer = (n - 2) ** 2
+    expect = np.zeros(3)
+    for k in range(19):
+        if c[k][2] == 1:
+            expect += nlayer * (-6.0 * t[k] * (c[k] @ uw)) * c[opp[k]]
+    assert np.abs(mom - expect).max() < 1e-13
+    assert expect[0] > 0
+
+
+# ------------------------------------------------------------------ P3: shear-wave decay
+
+def _shear_amplitude(oracle, Q, model, omega, steps, ny=128):
+    rho, u = inputs.shear_wave(1, ny, 1)
+    o = oracle.Oracle(1, ny, 1, Q, model, omega)
+    o.set_flags(np.zeros(ny, dtype=np.uint8))
+    o.init_equilibrium(rho, u)
+    s = np.sin(2 * np.pi * np.arange(ny) / ny)
+    a0 = 2.0 / ny * (o.macroscopic()[1][0] @ s)
+    e0 = o.kinetic_energy()
+    o.step(steps)
+    a1 = 2.0 / ny * (o.macroscopic()[1][0] @ s)
+    return a1 / a0, o.kinetic_energy() / e0
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_p3_shear_wave_omega_1(oracle, Q):
+    """nu = (1/omega - 1/2)/3 (L352): amplitude decays as exp(-nu k^2 t); tight at omega = 1."""
+    ny, steps = 128, 1000
+    k2 = (2 * np.pi / ny) ** 2
+    nu = (1 / 1.0 - 0.5) / 3
+    ratio, eratio = _shear_amplitude(oracle, Q, "BGK_W2", 1.0, steps)
+    nu_fit = -np.log(ratio) / (k2 * steps)
+    assert abs(nu_fit / nu - 1) < 1e-6
+    assert abs(eratio - np.exp(-2 * nu * k2 * steps)) < 1e-5       # R19: E ~ exp(-2 nu k^2 t)
+
+
+@pytest.mark.parametrize("model", ALL_MODELS)
+def test_p3_shear_wave_all_models_same_viscosity(oracle, model):
+    ny, steps, omega = 128, 400, 1.6
+    k2 = (2 * np.pi / ny) ** 2
+    nu = (1 / omega - 0.5) / 3
+    ratio, _ = _shear_amplitude(oracle, 19, model, omega, steps)
+    nu_fit = -np.log(ratio) / (k2 * steps)
+    assert abs(nu_fit / nu - 1) < 1e-2, (model, nu_fit, nu)
+
+
+def test_p3_shear_wave_config2_omega(oracle):
+    """At config 2's omega = 1.9702 the amplitude ratio after 1000 steps is within 5e-4 of exp(-nu k^2 t)."""
+    omega = inputs.omega_from_re(128, 1000)
+    assert abs(omega - 1.9702104184) < 1e-9
+    nu = (1 / omega - 0.5) / 3
+    ratio, _ = _shear_amplitude(oracle, 19, "BGK_W2", omega, 1000)
+    assert abs(ratio - np.exp(-nu * (2 * np.pi / 128) ** 2 * 1000)) < 5e-4
+
+
+# ------------------------------------------------------------------ P4: Poiseuille between bounce-back walls
+
+@pytest.mark.parametrize("model,lam", [("TRT", 3 / 16), ("TRT", 1 / 4), ("BGK_W2", None)])
+def test_p4_poiseuille_profile(oracle, model, lam):
+    """Half-way bounce-back (L92): u(y) = g/(2 nu) y (H - y) + g (16 Lambda - 3)/(24 nu), y from the
+    half-way wall; Lambda = 3/16 puts the wall exactly half-way, BGK has Lambda = (1/omega - 1/2)^2."""
+    H, omega, g = 8, 1.2, 1e-6
+    nu = (1 / omega - 0.5) / 3
+    ny = H + 2
+    fl = np.zeros((1, ny, 1), dtype=np.uint8)
+    fl[0, 0, 0] = fl[0, -1, 0] = inputs.WALL
+    o = oracle.Oracle(1, ny, 1, 19, model, omega)
+    o.set_flags(fl)
+    if lam is not None:
+        o.set_trt_magic(lam)
+    else:
+        lam = (1 / omega - 0.5) ** 2
+    o.set_force([g, 0.0, 0.0])
+    o.init_equilibrium(np.ones(ny), np.zeros((3, ny)))
+    o.step(3000)
+    ux = o.macroscopic()[1][0][1:-1]
+    y = np.arange(1, H + 1) - 0.5
+    expect = g / (2 * nu) * y * (H - y) + g * (16 * lam - 3) / (24 * nu)
+    assert np.abs(ux - expect).max() < 1e-9 * expect.max()
+
+
+# ------------------------------------------------------------------ config sanity (R11)
+
+def test_config_omegas():
+    assert abs(inputs.omega_from_re(32, 100) - 1.9305019305) < 1e-9
+    assert abs(inputs.omega_from_re(256, 1000) - 1.9408431023) < 1e-9
+    assert abs(inputs.omega_from_re(192, 1000) - 1.9554165037) < 1e-9
+    assert abs(inputs.omega_from_re(512, 1000) - 1.8846588768) < 1e-9
+
+
+def test_seeded_inputs_are_order_independent():
+    rho, u = inputs.seeded_init(4, 5, 6, seed=0)
+    idx = np.array([7, 3, 100])
+    r2, u2 = inputs.seeded_init(1, 1, 3, seed=0, index_offset=idx)
+    assert np.array_equal(r2, rho[idx]) and np.array_equal(u2, u[:, idx])
+    assert np.abs(rho - 1).max() <= 1e-3 and np.abs(u).max() <= 0.01
+    assert abs(rho.mean() - 1) < 2e-4 and np.unique(rho).size == rho.size
