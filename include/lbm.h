@@ -1,0 +1,113 @@
+/*
+ * lbm.h -- C ABI of the B200-native lattice Boltzmann stream-and-collide library
+ * (liblbm_b200.so), after arxiv 2010.11751 (Latt, Coreixas, Beny).  Citations "PAPER.md:Lnnn"
+ * are lines of the paper text; "R<n>" are the readings listed in DESIGN.md.
+ *
+ * Conventions shared by every call
+ *   - Host arrays are indexed i = (ix*ny + iy)*nz + iz, z fastest.
+ *     u is three planes [3][N]; populations are [Q][N] in the canonical direction order (R7):
+ *     D3Q19: k=0..8 = (-1,0,0),(0,-1,0),(0,0,-1),(-1,-1,0),(-1,1,0),(-1,0,-1),(-1,0,1),(0,-1,-1),
+ *     (0,-1,1); k=9 rest; k=10..18 their negatives.  D3Q27 appends (-1,-1,-1),(-1,-1,1),(-1,1,-1),
+ *     (-1,1,1) to the half set (rest at 13, opposite of k is k+14).  The internal device layout
+ *     (padding, AoS, AA shuffling, post-collision storage) is never visible.
+ *   - "host" pointers are caller-owned and only read / written during the call.  The context owns
+ *     every device buffer; device memory and the stream come from the hooks (lbm_set_hooks), which
+ *     the Python binding points at torch's caching allocator and current stream.
+ *   - Index arithmetic wraps periodically on all three axes; walls exist only where flags say so
+ *     (a cavity is a box whose outermost layer is flagged).
+ *   - Non-fluid cells export populations 0, rho 0, u 0.
+ *   - Return value: 0 ok; LBM_E_ARG (-1) bad argument / unsupported combination; LBM_E_ALLOC (-2);
+ *     LBM_E_CUDA (-3); LBM_E_STATE (-4) wrong state (e.g. step before init).  lbm_create returns
+ *     NULL on failure.  The message is available from lbm_last_error() (thread-local).  Nothing
+ *     throws or aborts across this boundary, and there is no CPU fallback of any kind.
+ *   - One context = one stream; calls on one context are not re-entrant.
+ */
+#ifndef LBM_B200_H
+#define LBM_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct lbm_ctx lbm_t;
+
+enum { LBM_D3Q19 = 19, LBM_D3Q27 = 27 };
+/* collision models: the paper's nine plus regularised BGK (R18) */
+enum { LBM_BGK_W2 = 0, LBM_BGK_NW4, LBM_TRT, LBM_RM, LBM_HM, LBM_CM, LBM_CHM, LBM_K, LBM_RR, LBM_REG, LBM_NUM_MODELS };
+/* memory-access schemes x layouts (Table 1) */
+enum { LBM_2POP_SOA = 0, LBM_2POP_AOS, LBM_SWAP_SOA, LBM_SWAP_AOS, LBM_AA_SOA, LBM_AA_AOS, LBM_NUM_SCHEMES };
+enum { LBM_F32 = 0, LBM_F64 = 1 };
+enum { LBM_FLUID = 0, LBM_WALL = 1, LBM_MOVING = 2 }; /* cell flags */
+enum { LBM_OK = 0, LBM_E_ARG = -1, LBM_E_ALLOC = -2, LBM_E_CUDA = -3, LBM_E_STATE = -4 };
+
+/* Device-memory and stream hooks (process-wide; set before lbm_create).  alloc returns a device
+ * pointer of at least `bytes` bytes aligned to 256 B or NULL; free releases it; stream is a
+ * cudaStream_t (as void*) on which every kernel and copy of contexts created afterwards runs.
+ * With no hooks set the library uses cudaMalloc/cudaFree and the legacy default stream. */
+typedef void* (*lbm_alloc_fn)(size_t bytes);
+typedef void (*lbm_free_fn)(void* ptr);
+int lbm_set_hooks(lbm_alloc_fn alloc, lbm_free_fn free_fn, void* stream);
+
+/* Create a context for an nx*ny*nz box (each >= 3), lattice LBM_D3Q19|LBM_D3Q27, a collision
+ * model, a scheme, the shear relaxation rate omega in (0,2) with nu = (1/omega - 1/2)/3
+ * and the storage/arithmetic type.  All cells start FLUID (fully periodic box).
+ * Default rates (R14): omega_bulk = omega, moments of order >= 3 relaxed with 1 (RR: with omega);
+ * TRT magic parameter 1/4 (R15).  LBM_F32 is available for BGK_W2, TRT and REG. */
+lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme, double omega, int dtype);
+int lbm_destroy(lbm_t* ctx);
+
+/* Cell flags (host, uint8 [N]) and the velocity of LBM_MOVING cells (host double[3], may be NULL
+ * = 0).  Half-way bounce-back with the momentum term -6 t_k rho_w c_k.u_w, rho_w = 1, Eq 3
+ * (PAPER.md:L87-92).  Must precede lbm_init_equilibrium / lbm_set_populations. */
+int lbm_set_flags(lbm_t* ctx, const uint8_t* flags, const double u_wall[3]);
+
+/* Override the rates of Eq 11 / Eq 13-15: bulk rate, rate of third-order
+ * moments, rate of moments of order >= 4.  Ignored by BGK_W2, BGK_NW4, TRT and REG. */
+int lbm_set_relaxation(lbm_t* ctx, double omega_bulk, double omega3, double omega_hi);
+/* TRT magic parameter Lambda = (1/w+ - 1/2)(1/w- - 1/2) (default 1/4). */
+int lbm_set_trt_magic(lbm_t* ctx, double lambda);
+
+/* Fill every fluid cell with the model's own equilibrium (Eq 6 for BGK_W2/TRT/REG, the extended
+ * product-form equilibrium for the rest) of the given rho [N] and u [3][N]: host arrays of the
+ * context dtype.  Resets the step count and the AA parity. */
+int lbm_init_equilibrium(lbm_t* ctx, const void* rho, const void* u);
+
+/* n collide-and-stream cycles (Eq 1-3) by the context's scheme; asynchronous on
+ * the stream.  n >= 0. */
+int lbm_step(lbm_t* ctx, int n);
+
+/* rho = sum_k f_k, u = sum_k c_k f_k / rho per cell of the pre-collision
+ * populations at the current time; host outputs of the context dtype; synchronises. */
+int lbm_macroscopic(lbm_t* ctx, void* rho, void* u);
+
+/* E = sum over fluid cells of 1/2 rho |u|^2 (R19), accumulated in double with a fixed reduction
+ * tree (bitwise repeatable); synchronises. */
+int lbm_kinetic_energy(lbm_t* ctx, double* e);
+
+/* Pre-collision populations at the current time, canonical [Q][N] order, context dtype, host. */
+int lbm_get_populations(lbm_t* ctx, void* f);
+/* Load populations (same format); resets the AA parity to even. */
+int lbm_set_populations(lbm_t* ctx, const void* f);
+
+/* Introspection used by the harness: number of time steps done; number of fluid cells; bytes of
+ * device memory held; number of kernels launched by this context so far. */
+long long lbm_steps_done(const lbm_t* ctx);
+long long lbm_num_fluid(const lbm_t* ctx);
+long long lbm_device_bytes(const lbm_t* ctx);
+long long lbm_kernel_launches(const lbm_t* ctx);
+/* Block until everything queued on the context's stream has finished. */
+int lbm_sync(lbm_t* ctx);
+/* Select an implementation variant of the step kernels (0 = default); used by the bench sweep.
+ * Unknown variants return LBM_E_ARG.  Results are identical across variants. */
+int lbm_set_variant(lbm_t* ctx, int variant);
+
+const char* lbm_last_error(void);
+const char* lbm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LBM_B200_H */

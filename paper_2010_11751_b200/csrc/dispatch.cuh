@@ -1,0 +1,56 @@
+// dispatch.cuh -- host-side launch entry points shared by lbm_api.cu (caller), inst.cu (one object
+// per lattice x collision model: the step kernels) and aux.cu (model-independent kernels).
+#pragma once
+#include <cuda_runtime.h>
+#include "kernels.cuh"
+
+namespace lbm {
+
+// step-kernel kinds = (load mode, store mode) pairs, see kernels.cuh
+enum StepKind {
+    SK_PUSH = 0,   // LD_LOCAL  -> ST_PUSH     two-population, collide then push (Table 1)
+    SK_PULL,       // LD_PULL   -> ST_LOCAL    two-population, pull then collide (post-collision storage)
+    SK_COLLIDE,    // LD_LOCAL  -> ST_LOCAL    collide only (first step of the pull form)
+    SK_EVEN,       // LD_LOCAL  -> ST_SWAPPED  AA even step / swap pass 1 (Table 1)
+    SK_ODD,        // LD_AAPULL -> ST_PUSH     AA odd step (Table 1)
+    SK_COUNT
+};
+
+// implementation variants of the step kernels (lbm_set_variant)
+enum Variant {
+    V_DEFAULT = 0,   // library's choice
+    V_GENERIC_PUSH,  // generic one-thread-per-cell kernels, 2-pop as collide-then-push
+    V_GENERIC_PULL,  // generic kernels, 2-pop as pull-then-collide with lazily streamed storage
+    V_COUNT
+};
+
+// defined in inst.cu, explicitly instantiated once per (T, Q, MODEL)
+template <class T, int Q, int MODEL>
+cudaError_t launch_step(int kind, bool soa, int block, const StepArgs<T>& a, cudaStream_t s);
+
+// defined in aux.cu
+cudaError_t aux_classify(const uint8_t* flags, uint8_t* code, const Geo& g, cudaStream_t s);
+template <class T>
+cudaError_t aux_init_equilibrium(int Q, bool ext, bool soa, T* pop, const uint8_t* code, const Geo& g, const T* rho,
+                                 const T* u, cudaStream_t s);
+template <class T>
+cudaError_t aux_macroscopic(int Q, bool soa, int load, const StepArgs<T>& a, T* rho, T* u, cudaStream_t s);
+template <class T>
+cudaError_t aux_energy(int Q, bool soa, int load, const StepArgs<T>& a, double* partial, int nblocks, double* out,
+                       cudaStream_t s);
+template <class T>
+cudaError_t aux_extract_plane(int Q, bool soa, const T* pop, const uint8_t* code, const Geo& g, const PlaneArgs& p,
+                              T* out, cudaStream_t s);
+template <class T>
+cudaError_t aux_insert_plane(int Q, bool soa, T* pop, const uint8_t* code, const Geo& g, int k, double weight,
+                             const T* in, cudaStream_t s);
+template <class T>
+cudaError_t aux_swap_stream(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s);
+// stream only (LD_PULL -> ST_LOCAL without collision): turns post-collision storage into canonical
+template <class T>
+cudaError_t aux_stream_only(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s);
+
+// host copies of the lattice tables (from Lat<Q>)
+void lattice_tables(int Q, int (*c)[3], int* opp, double* w);
+
+}  // namespace lbm

@@ -1,0 +1,480 @@
+// lbm_api.cu -- the C ABI of include/lbm.h: context, state machine of the schemes, argument
+// checks and kernel launches.  No arithmetic of the method lives here; every step of the path
+// runs in the kernels of kernels.cuh / fast19.cuh.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "../../include/lbm.h"
+#include "dispatch.cuh"
+
+using namespace lbm;
+
+namespace {
+
+thread_local char g_err[512] = "";
+void set_err(const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+
+lbm_alloc_fn g_alloc = nullptr;
+lbm_free_fn g_free = nullptr;
+cudaStream_t g_stream = nullptr;
+
+enum Family { FAM_2POP, FAM_SWAP, FAM_AA };
+// where the pre-collision state of the current time lives
+enum Storage {
+    STO_NONE,      // nothing loaded yet
+    STO_CANON,     // pop_k(x) = f_k(x)                      (LD_LOCAL)
+    STO_POST,      // pop holds f_out of the previous step   (LD_PULL), 2-pop pull form
+    STO_AA_ODD     // after an AA even step                  (LD_AAPULL)
+};
+
+}  // namespace
+
+struct lbm_ctx {
+    int nx, ny, nz, Q, model, scheme, dtype;
+    Family fam;
+    bool soa;
+    double omega, omega_bulk, omega3, omega_hi, trt_magic;
+    double u_wall[3];
+    Geo g;
+    size_t elem;        // bytes per population
+    size_t pop_elems;   // elements in one population array
+    void* pop[2];       // [1] only for FAM_2POP
+    uint8_t* code;
+    void* scratch;      // 4 planes of N elements (rho,u staging; plane import/export)
+    double* partial;    // energy partial sums
+    double* e_dev;
+    int n_partial;
+    Storage sto;
+    int variant;
+    int block;
+    long long steps, launches, dev_bytes, n_fluid;
+    lbm_alloc_fn alloc;
+    lbm_free_fn free_fn;
+    cudaStream_t stream;
+    int c[27][3], opp[27];
+    double w[27];
+};
+
+namespace {
+
+void* dev_alloc(lbm_ctx* c, size_t bytes)
+{
+    void* p = nullptr;
+    if (c->alloc) p = c->alloc(bytes);
+    else if (cudaMalloc(&p, bytes) != cudaSuccess) p = nullptr;
+    if (p) c->dev_bytes += (long long)bytes;
+    return p;
+}
+void dev_free(lbm_ctx* c, void* p)
+{
+    if (!p) return;
+    if (c->free_fn) c->free_fn(p);
+    else cudaFree(p);
+}
+
+int cuda_fail(const char* what, cudaError_t e)
+{
+    set_err("%s: %s", what, cudaGetErrorString(e));
+    return LBM_E_CUDA;
+}
+#define CK(call)                                         \
+    do {                                                 \
+        cudaError_t e_ = (call);                         \
+        if (e_ != cudaSuccess) return cuda_fail(#call, e_); \
+    } while (0)
+
+template <class T>
+StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst)
+{
+    StepArgs<T> a;
+    a.src = (const T*)src;
+    a.dst = (T*)dst;
+    a.code = c->code;
+    a.g = c->g;
+    a.rt.omega = (T)c->omega;
+    a.rt.omega_bulk = (T)c->omega_bulk;
+    a.rt.omega3 = (T)c->omega3;
+    a.rt.omega_hi = (T)c->omega_hi;
+    // TRT: Lambda = (1/w+ - 1/2)(1/w- - 1/2)
+    a.rt.omega_minus = (T)(1.0 / (c->trt_magic / (1.0 / c->omega - 0.5) + 0.5));
+    for (int k = 0; k < 27; ++k) {
+        double cu = 0.0;
+        if (k < c->Q) cu = c->c[k][0] * c->u_wall[0] + c->c[k][1] * c->u_wall[1] + c->c[k][2] * c->u_wall[2];
+        a.wterm[k] = k < c->Q ? (T)(-6.0 * c->w[k] * cu) : (T)0;  // Eq 3, rho_w = 1
+    }
+    return a;
+}
+
+template <class T, int Q>
+cudaError_t step_model(const lbm_ctx* c, int kind, const StepArgs<T>& a)
+{
+    const bool soa = c->soa;
+    const int b = c->block;
+    cudaStream_t s = c->stream;
+    switch (c->model) {
+    case LBM_BGK_W2: return launch_step<T, Q, M_BGK_W2>(kind, soa, b, a, s);
+    case LBM_TRT: return launch_step<T, Q, M_TRT>(kind, soa, b, a, s);
+    case LBM_REG: return launch_step<T, Q, M_REG>(kind, soa, b, a, s);
+    default: break;
+    }
+    if constexpr (sizeof(T) == 8) {
+        switch (c->model) {
+        case LBM_BGK_NW4: return launch_step<T, Q, M_BGK_NW4>(kind, soa, b, a, s);
+        case LBM_RM: return launch_step<T, Q, M_RM>(kind, soa, b, a, s);
+        case LBM_HM: return launch_step<T, Q, M_HM>(kind, soa, b, a, s);
+        case LBM_CM: return launch_step<T, Q, M_CM>(kind, soa, b, a, s);
+        case LBM_CHM: return launch_step<T, Q, M_CHM>(kind, soa, b, a, s);
+        case LBM_K: return launch_step<T, Q, M_K>(kind, soa, b, a, s);
+        case LBM_RR: return launch_step<T, Q, M_RR>(kind, soa, b, a, s);
+        default: break;
+        }
+    }
+    return cudaErrorInvalidValue;
+}
+
+template <class T>
+cudaError_t step_kind(lbm_ctx* c, int kind, const void* src, void* dst)
+{
+    StepArgs<T> a = make_args<T>(c, src, dst);
+    c->launches++;
+    return c->Q == 19 ? step_model<T, 19>(c, kind, a) : step_model<T, 27>(c, kind, a);
+}
+cudaError_t step_kind(lbm_ctx* c, int kind, const void* src, void* dst)
+{
+    return c->dtype == LBM_F64 ? step_kind<double>(c, kind, src, dst) : step_kind<float>(c, kind, src, dst);
+}
+
+int load_mode(const lbm_ctx* c)
+{
+    return c->sto == STO_POST ? LD_PULL : c->sto == STO_AA_ODD ? LD_AAPULL : LD_LOCAL;
+}
+
+bool use_pull(const lbm_ctx* c) { return c->variant == V_GENERIC_PULL; }
+
+// bring post-collision 2-pop storage back to canonical (one stream-only pass)
+int normalise(lbm_ctx* c)
+{
+    if (c->sto != STO_POST) return LBM_OK;
+    cudaError_t e;
+    if (c->dtype == LBM_F64) e = aux_stream_only<double>(c->Q, c->soa, make_args<double>(c, c->pop[0], c->pop[1]), c->stream);
+    else e = aux_stream_only<float>(c->Q, c->soa, make_args<float>(c, c->pop[0], c->pop[1]), c->stream);
+    c->launches++;
+    if (e != cudaSuccess) return cuda_fail("stream_only", e);
+    void* t = c->pop[0]; c->pop[0] = c->pop[1]; c->pop[1] = t;
+    c->sto = STO_CANON;
+    return LBM_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* lbm_last_error(void) { return g_err; }
+const char* lbm_version(void) { return "lbm_b200 0.1 (sm_100a)"; }
+
+int lbm_set_hooks(lbm_alloc_fn alloc, lbm_free_fn free_fn, void* stream)
+{
+    if ((alloc == nullptr) != (free_fn == nullptr)) { set_err("alloc and free hooks must be given together"); return LBM_E_ARG; }
+    g_alloc = alloc;
+    g_free = free_fn;
+    g_stream = (cudaStream_t)stream;
+    return LBM_OK;
+}
+
+lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme, double omega, int dtype)
+{
+    if (nx < 3 || ny < 3 || nz < 3) { set_err("extents must be >= 3 (got %d %d %d)", nx, ny, nz); return nullptr; }
+    if ((long long)nx * ny * nz >= (1LL << 31) - 64) { set_err("too many cells"); return nullptr; }
+    if (lattice != LBM_D3Q19 && lattice != LBM_D3Q27) { set_err("lattice must be 19 or 27"); return nullptr; }
+    if (collision < 0 || collision >= LBM_NUM_MODELS) { set_err("unknown collision model %d", collision); return nullptr; }
+    if (scheme < 0 || scheme >= LBM_NUM_SCHEMES) { set_err("unknown scheme %d", scheme); return nullptr; }
+    if (dtype != LBM_F32 && dtype != LBM_F64) { set_err("dtype must be LBM_F32 or LBM_F64"); return nullptr; }
+    if (!(omega > 0.0 && omega < 2.0)) { set_err("omega must be in (0,2)"); return nullptr; }
+    if (dtype == LBM_F32 && !model_is_w2(collision)) {
+        set_err("fp32 is available for BGK_W2, TRT and REG only");
+        return nullptr;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        set_err("no CUDA device: this library has no CPU fallback");
+        return nullptr;
+    }
+    lbm_ctx* c = new (std::nothrow) lbm_ctx();
+    if (!c) { set_err("out of host memory"); return nullptr; }
+    memset(c, 0, sizeof *c);
+    c->nx = nx; c->ny = ny; c->nz = nz; c->Q = lattice; c->model = collision; c->scheme = scheme; c->dtype = dtype;
+    c->fam = (scheme == LBM_2POP_SOA || scheme == LBM_2POP_AOS) ? FAM_2POP
+           : (scheme == LBM_SWAP_SOA || scheme == LBM_SWAP_AOS) ? FAM_SWAP : FAM_AA;
+    c->soa = scheme == LBM_2POP_SOA || scheme == LBM_SWAP_SOA || scheme == LBM_AA_SOA;
+    c->omega = omega;
+    c->omega_bulk = omega;                                   // R14
+    c->omega3 = collision == LBM_RR ? omega : 1.0;           // R14
+    c->omega_hi = collision == LBM_RR ? omega : 1.0;
+    c->trt_magic = 0.25;                                     // R15
+    c->elem = dtype == LBM_F64 ? 8 : 4;
+    c->g.nx = nx; c->g.ny = ny; c->g.nz = nz; c->g.n = nx * ny * nz;
+    const long long per128 = 128 / (long long)c->elem;
+    c->g.stride = ((long long)c->g.n + per128 - 1) / per128 * per128;  // planes start 128 B aligned
+    c->pop_elems = c->soa ? (size_t)c->g.stride * c->Q : (size_t)c->g.n * c->Q;
+    c->alloc = g_alloc; c->free_fn = g_free; c->stream = g_stream;
+    c->variant = V_DEFAULT;
+    c->block = 128;
+    c->n_fluid = c->g.n;
+    lattice_tables(c->Q, c->c, c->opp, c->w);
+
+    const int narr = c->fam == FAM_2POP ? 2 : 1;
+    bool ok = true;
+    for (int a = 0; a < narr && ok; ++a) {
+        c->pop[a] = dev_alloc(c, c->pop_elems * c->elem);
+        ok = c->pop[a] != nullptr;
+        if (ok) ok = cudaMemsetAsync(c->pop[a], 0, c->pop_elems * c->elem, c->stream) == cudaSuccess;
+    }
+    if (ok) { c->code = (uint8_t*)dev_alloc(c, (size_t)c->g.n); ok = c->code != nullptr; }
+    if (ok) ok = cudaMemsetAsync(c->code, 0, (size_t)c->g.n, c->stream) == cudaSuccess;
+    if (ok) { c->scratch = dev_alloc(c, 4 * (size_t)c->g.n * c->elem); ok = c->scratch != nullptr; }
+    c->n_partial = 148 * 8;
+    if (ok) { c->partial = (double*)dev_alloc(c, sizeof(double) * (c->n_partial + 1)); ok = c->partial != nullptr; }
+    if (!ok) {
+        set_err("device allocation failed (%lld bytes so far): %s", c->dev_bytes, cudaGetErrorString(cudaGetLastError()));
+        lbm_destroy(c);
+        return nullptr;
+    }
+    c->e_dev = c->partial + c->n_partial;
+    // cells on the faces of a fully periodic box still need the wrap: classify with all-fluid flags
+    // (scratch is large enough to stand in for a zero flag array of N bytes)
+    if (cudaMemsetAsync(c->scratch, 0, (size_t)c->g.n, c->stream) != cudaSuccess ||
+        aux_classify((const uint8_t*)c->scratch, c->code, c->g, c->stream) != cudaSuccess) {
+        set_err("classification launch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        lbm_destroy(c);
+        return nullptr;
+    }
+    c->launches++;
+    return c;
+}
+
+int lbm_destroy(lbm_t* c)
+{
+    if (!c) return LBM_OK;
+    cudaStreamSynchronize(c->stream);
+    dev_free(c, c->pop[0]);
+    dev_free(c, c->pop[1]);
+    dev_free(c, c->code);
+    dev_free(c, c->scratch);
+    dev_free(c, c->partial);
+    delete c;
+    return LBM_OK;
+}
+
+int lbm_set_flags(lbm_t* c, const uint8_t* flags, const double u_wall[3])
+{
+    if (!c || !flags) { set_err("null argument"); return LBM_E_ARG; }
+    long long nfluid = 0;
+    for (int i = 0; i < c->g.n; ++i) {
+        if (flags[i] > LBM_MOVING) { set_err("flag %d at cell %d is not FLUID/WALL/MOVING", flags[i], i); return LBM_E_ARG; }
+        nfluid += flags[i] == LBM_FLUID;
+    }
+    for (int a = 0; a < 3; ++a) c->u_wall[a] = u_wall ? u_wall[a] : 0.0;
+    CK(cudaMemcpyAsync(c->scratch, flags, (size_t)c->g.n, cudaMemcpyHostToDevice, c->stream));
+    CK(aux_classify((const uint8_t*)c->scratch, c->code, c->g, c->stream));
+    c->launches++;
+    CK(cudaStreamSynchronize(c->stream));
+    c->n_fluid = nfluid;
+    c->sto = STO_NONE;  // populations of cells that changed type are meaningless now
+    return LBM_OK;
+}
+
+int lbm_set_relaxation(lbm_t* c, double omega_bulk, double omega3, double omega_hi)
+{
+    if (!c) { set_err("null context"); return LBM_E_ARG; }
+    if (!(omega_bulk > 0.0 && omega_bulk < 2.0) || !(omega3 > 0.0 && omega3 < 2.0) || !(omega_hi > 0.0 && omega_hi < 2.0)) {
+        set_err("relaxation rates must be in (0,2)");
+        return LBM_E_ARG;
+    }
+    c->omega_bulk = omega_bulk; c->omega3 = omega3; c->omega_hi = omega_hi;
+    return LBM_OK;
+}
+
+int lbm_set_trt_magic(lbm_t* c, double lambda)
+{
+    if (!c || !(lambda > 0.0)) { set_err("magic parameter must be positive"); return LBM_E_ARG; }
+    c->trt_magic = lambda;
+    return LBM_OK;
+}
+
+int lbm_init_equilibrium(lbm_t* c, const void* rho, const void* u)
+{
+    if (!c || !rho || !u) { set_err("null argument"); return LBM_E_ARG; }
+    const size_t nb = (size_t)c->g.n * c->elem;
+    char* sc = (char*)c->scratch;
+    CK(cudaMemcpyAsync(sc, rho, nb, cudaMemcpyHostToDevice, c->stream));
+    CK(cudaMemcpyAsync(sc + nb, u, 3 * nb, cudaMemcpyHostToDevice, c->stream));
+    const bool ext = !model_is_w2(c->model);
+    if (c->dtype == LBM_F64)
+        CK(aux_init_equilibrium<double>(c->Q, ext, c->soa, (double*)c->pop[0], c->code, c->g, (const double*)sc,
+                                        (const double*)(sc + nb), c->stream));
+    else
+        CK(aux_init_equilibrium<float>(c->Q, ext, c->soa, (float*)c->pop[0], c->code, c->g, (const float*)sc,
+                                       (const float*)(sc + nb), c->stream));
+    c->launches++;
+    CK(cudaStreamSynchronize(c->stream));  // host buffers are only read during the call
+    c->sto = STO_CANON;
+    c->steps = 0;
+    return LBM_OK;
+}
+
+int lbm_step(lbm_t* c, int n)
+{
+    if (!c) { set_err("null context"); return LBM_E_ARG; }
+    if (n < 0) { set_err("n must be >= 0"); return LBM_E_ARG; }
+    if (c->sto == STO_NONE) { set_err("lbm_step before lbm_init_equilibrium / lbm_set_populations"); return LBM_E_STATE; }
+    for (int s = 0; s < n; ++s) {
+        if (c->fam == FAM_2POP) {
+            if (use_pull(c)) {
+                if (c->sto == STO_CANON) {  // (S C)^n = S (C S)^(n-1) C: start with a collide-only pass
+                    CK(step_kind(c, SK_COLLIDE, c->pop[0], c->pop[0]));
+                    c->sto = STO_POST;
+                } else {
+                    CK(step_kind(c, SK_PULL, c->pop[0], c->pop[1]));
+                    void* t = c->pop[0]; c->pop[0] = c->pop[1]; c->pop[1] = t;
+                }
+            } else {
+                if (int rc = normalise(c)) return rc;
+                CK(step_kind(c, SK_PUSH, c->pop[0], c->pop[1]));
+                void* t = c->pop[0]; c->pop[0] = c->pop[1]; c->pop[1] = t;
+            }
+        } else if (c->fam == FAM_AA) {
+            if (c->sto == STO_CANON) {
+                CK(step_kind(c, SK_EVEN, c->pop[0], c->pop[0]));
+                c->sto = STO_AA_ODD;
+            } else {
+                CK(step_kind(c, SK_ODD, c->pop[0], c->pop[0]));
+                c->sto = STO_CANON;
+            }
+        } else {
+            CK(step_kind(c, SK_EVEN, c->pop[0], c->pop[0]));  // pass 1: collide into opposite slots
+            if (c->dtype == LBM_F64) CK(aux_swap_stream<double>(c->Q, c->soa, make_args<double>(c, c->pop[0], c->pop[0]), c->stream));
+            else CK(aux_swap_stream<float>(c->Q, c->soa, make_args<float>(c, c->pop[0], c->pop[0]), c->stream));
+            c->launches++;
+        }
+        c->steps++;
+    }
+    return LBM_OK;
+}
+
+int lbm_macroscopic(lbm_t* c, void* rho, void* u)
+{
+    if (!c || !rho || !u) { set_err("null argument"); return LBM_E_ARG; }
+    if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
+    const size_t nb = (size_t)c->g.n * c->elem;
+    char* sc = (char*)c->scratch;
+    if (c->dtype == LBM_F64)
+        CK(aux_macroscopic<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr), (double*)sc,
+                                   (double*)(sc + nb), c->stream));
+    else
+        CK(aux_macroscopic<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr), (float*)sc,
+                                  (float*)(sc + nb), c->stream));
+    c->launches++;
+    CK(cudaMemcpyAsync(rho, sc, nb, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaMemcpyAsync(u, sc + nb, 3 * nb, cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return LBM_OK;
+}
+
+int lbm_kinetic_energy(lbm_t* c, double* e)
+{
+    if (!c || !e) { set_err("null argument"); return LBM_E_ARG; }
+    if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
+    if (c->dtype == LBM_F64)
+        CK(aux_energy<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr), c->partial,
+                              c->n_partial, c->e_dev, c->stream));
+    else
+        CK(aux_energy<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr), c->partial,
+                             c->n_partial, c->e_dev, c->stream));
+    c->launches += 2;
+    CK(cudaMemcpyAsync(e, c->e_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    CK(cudaStreamSynchronize(c->stream));
+    return LBM_OK;
+}
+
+int lbm_get_populations(lbm_t* c, void* f)
+{
+    if (!c || !f) { set_err("null argument"); return LBM_E_ARG; }
+    if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
+    const size_t nb = (size_t)c->g.n * c->elem;
+    const int mode = load_mode(c);
+    // two scratch planes alternate so that the copy of plane k overlaps nothing it still needs
+    for (int k = 0; k < c->Q; ++k) {
+        const int kb = c->opp[k];
+        PlaneArgs p;
+        p.weight = c->w[k];
+        const double cu = c->c[kb][0] * c->u_wall[0] + c->c[kb][1] * c->u_wall[1] + c->c[kb][2] * c->u_wall[2];
+        p.wterm = -6.0 * c->w[kb] * cu;
+        if (mode == LD_LOCAL) { p.slot_fluid = k; p.slot_wall = k; p.sx = p.sy = p.sz = 0; }
+        else {
+            p.slot_fluid = mode == LD_PULL ? k : kb;
+            p.slot_wall = mode == LD_PULL ? kb : k;
+            p.sx = c->c[k][0]; p.sy = c->c[k][1]; p.sz = c->c[k][2];
+        }
+        char* out = (char*)c->scratch + (size_t)(k & 3) * nb;
+        if (c->dtype == LBM_F64)
+            CK(aux_extract_plane<double>(c->Q, c->soa, (const double*)c->pop[0], c->code, c->g, p, (double*)out, c->stream));
+        else
+            CK(aux_extract_plane<float>(c->Q, c->soa, (const float*)c->pop[0], c->code, c->g, p, (float*)out, c->stream));
+        c->launches++;
+        CK(cudaMemcpyAsync((char*)f + (size_t)k * nb, out, nb, cudaMemcpyDeviceToHost, c->stream));
+    }
+    CK(cudaStreamSynchronize(c->stream));
+    return LBM_OK;
+}
+
+int lbm_set_populations(lbm_t* c, const void* f)
+{
+    if (!c || !f) { set_err("null argument"); return LBM_E_ARG; }
+    const size_t nb = (size_t)c->g.n * c->elem;
+    for (int k = 0; k < c->Q; ++k) {
+        char* in = (char*)c->scratch + (size_t)(k & 3) * nb;
+        CK(cudaMemcpyAsync(in, (const char*)f + (size_t)k * nb, nb, cudaMemcpyHostToDevice, c->stream));
+        if (c->dtype == LBM_F64)
+            CK(aux_insert_plane<double>(c->Q, c->soa, (double*)c->pop[0], c->code, c->g, k, c->w[k], (const double*)in, c->stream));
+        else
+            CK(aux_insert_plane<float>(c->Q, c->soa, (float*)c->pop[0], c->code, c->g, k, c->w[k], (const float*)in, c->stream));
+        c->launches++;
+    }
+    CK(cudaStreamSynchronize(c->stream));
+    c->sto = STO_CANON;
+    return LBM_OK;
+}
+
+long long lbm_steps_done(const lbm_t* c) { return c ? c->steps : -1; }
+long long lbm_num_fluid(const lbm_t* c) { return c ? c->n_fluid : -1; }
+long long lbm_device_bytes(const lbm_t* c) { return c ? c->dev_bytes : -1; }
+long long lbm_kernel_launches(const lbm_t* c) { return c ? c->launches : -1; }
+
+int lbm_sync(lbm_t* c)
+{
+    if (!c) { set_err("null context"); return LBM_E_ARG; }
+    CK(cudaStreamSynchronize(c->stream));
+    return LBM_OK;
+}
+
+int lbm_set_variant(lbm_t* c, int variant)
+{
+    if (!c) { set_err("null context"); return LBM_E_ARG; }
+    if (variant < 0 || variant >= V_COUNT) { set_err("unknown variant %d", variant); return LBM_E_ARG; }
+    if (c->fam == FAM_2POP && variant != V_GENERIC_PULL) {
+        if (int rc = normalise(c)) return rc;
+    }
+    c->variant = variant;
+    return LBM_OK;
+}
+
+}  // extern "C"

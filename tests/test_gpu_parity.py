@@ -1,0 +1,173 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Tolerances are BASELINE.json's: max-abs population difference <= 1e-12
+after 100 steps in fp64; <= 2e-5 relative (to max(|f|, t_k), reading R20) in fp32."""
+import numpy as np
+import pytest
+
+from paper_2010_11751_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12
+TOL32 = 2e-5
+ALL_MODELS = ["BGK_W2", "BGK_NW4", "TRT", "RM", "HM", "CM", "CHM", "K", "RR", "REG"]
+ALL_SCHEMES = ["2POP_SOA", "2POP_AOS", "SWAP_SOA", "SWAP_AOS", "AA_SOA", "AA_AOS"]
+
+
+@pytest.fixture(scope="module")
+def Lbm():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2010_11751_b200 import Lbm as cls
+    return cls
+
+
+def box_flags(nx, ny, nz, kind):
+    if kind == "cavity":
+        return inputs.cavity_flags(nx, ny, nz), (inputs.U_LID, 0.0, 0.0)
+    if kind == "periodic":
+        return inputs.periodic_flags(nx, ny, nz), (0.0, 0.0, 0.0)
+    if kind == "obstacle":  # periodic box with a moving block and a resting block inside: walls + seam
+        fl = inputs.periodic_flags(nx, ny, nz)
+        fl[1:3, 2:4, 1:3] = inputs.MOVING
+        fl[nx - 2:, 0:2, nz // 2] = inputs.WALL
+        return fl, (0.01, -0.02, 0.015)
+    raise ValueError(kind)
+
+
+def run_pair(Lbm, oracle, shape, Q, model, scheme, dtype, steps, kind="cavity", omega=1.7, variant=None, seed=0,
+             rates=None, chunks=None):
+    nx, ny, nz = shape
+    fl, uw = box_flags(nx, ny, nz, kind)
+    rho, u = inputs.seeded_init(nx, ny, nz, seed)
+    npdt = np.float32 if dtype == "f32" else np.float64
+    rho_in, u_in = rho.astype(npdt), u.astype(npdt)
+    g = Lbm(nx, ny, nz, lattice=Q, collision=model, scheme=scheme, omega=omega, dtype=dtype)
+    o = oracle.Oracle(nx, ny, nz, Q=Q, model=model, omega=omega)
+    g.set_flags(fl, uw)
+    o.set_flags(fl, uw)
+    if rates is not None:
+        g.set_relaxation(*rates)
+        o.set_relaxation(*rates)
+    if variant is not None:
+        g.set_variant(variant)
+    g.init_equilibrium(rho_in, u_in)
+    o.init_equilibrium(rho_in.astype(np.float64), u_in.astype(np.float64))  # oracle fed the rounded inputs (R20)
+    for n in (chunks or [steps]):
+        g.step(n)
+    o.step(steps)
+    assert g.steps_done == steps
+    return g, o, fl
+
+
+def pop_error(g, o, fl, Q, oracle, relative):
+    fg = g.get_populations().astype(np.float64)
+    fo = o.get_populations()
+    assert np.isfinite(fg).all()
+    fluid = (fl.reshape(-1) == 0)
+    assert np.all(fg[:, ~fluid] == 0.0)
+    d = np.abs(fg - fo)[:, fluid]
+    if not relative:
+        return d.max()
+    _, t, _, _ = oracle.lattice(Q)
+    den = np.maximum(np.abs(fo[:, fluid]), t[:, None])
+    return (d / den).max()
+
+
+def test_config1_cavity32_bgk_2pop_fp64(Lbm, oracle):
+    """BASELINE.json config 1: 32^3 cavity, D3Q19 BGK-W2, 2-pop SoA, Re=100, 100 steps."""
+    n = 32
+    omega = inputs.omega_from_re(n, 100)
+    g, o, fl = run_pair(Lbm, oracle, (n, n, n), 19, "BGK_W2", "2POP_SOA", "f64", 100, omega=omega)
+    err = pop_error(g, o, fl, 19, oracle, False)
+    assert err <= TOL64, err
+    rg, ug = g.macroscopic()
+    ro, uo = o.macroscopic()
+    assert np.abs(rg - ro).max() <= 1e-12 and np.abs(ug - uo).max() <= 1e-12
+    eg, eo = g.kinetic_energy(), o.kinetic_energy()
+    assert abs(eg - eo) <= 1e-12 * max(1.0, abs(eo))
+    assert eg == g.kinetic_energy()  # fixed reduction tree: bitwise repeatable
+
+
+@pytest.mark.parametrize("variant", ["generic_push", "generic_pull"])
+@pytest.mark.parametrize("kind", ["cavity", "periodic", "obstacle"])
+def test_2pop_variants_ragged(Lbm, oracle, variant, kind):
+    g, o, fl = run_pair(Lbm, oracle, (13, 10, 7), 19, "BGK_W2", "2POP_SOA", "f64", 25, kind=kind, variant=variant,
+                        chunks=[1, 7, 17])
+    assert pop_error(g, o, fl, 19, oracle, False) <= TOL64
+    rg, ug = g.macroscopic()
+    ro, uo = o.macroscopic()
+    assert np.abs(rg - ro).max() <= 1e-12 and np.abs(ug - uo).max() <= 1e-12
+    assert abs(g.kinetic_energy() - o.kinetic_energy()) <= 1e-13
+
+
+@pytest.mark.parametrize("Q", [19, 27])
+@pytest.mark.parametrize("scheme", ALL_SCHEMES)
+@pytest.mark.parametrize("kind", ["cavity", "obstacle"])
+def test_schemes_match_oracle(Lbm, oracle, Q, scheme, kind):
+    """all six schemes give the oracle's populations, at even and odd step counts"""
+    for steps in (6, 7):
+        g, o, fl = run_pair(Lbm, oracle, (9, 11, 8), Q, "BGK_W2", scheme, "f64", steps, kind=kind)
+        assert pop_error(g, o, fl, Q, oracle, False) <= TOL64
+        rg, ug = g.macroscopic()
+        ro, uo = o.macroscopic()
+        assert np.abs(rg - ro).max() <= 1e-12 and np.abs(ug - uo).max() <= 1e-12
+        assert abs(g.kinetic_energy() - o.kinetic_energy()) <= 1e-13
+
+
+@pytest.mark.parametrize("Q", [19, 27])
+@pytest.mark.parametrize("model", ALL_MODELS)
+def test_models_match_oracle_100_steps(Lbm, oracle, Q, model):
+    """every collision model, default rates (R14), 100 steps on a small lid cavity, AA scheme"""
+    g, o, fl = run_pair(Lbm, oracle, (8, 9, 10), Q, model, "AA_SOA", "f64", 100, omega=1.6)
+    assert pop_error(g, o, fl, Q, oracle, False) <= TOL64
+
+
+@pytest.mark.parametrize("Q", [19, 27])
+@pytest.mark.parametrize("model", ["RM", "HM", "CM", "CHM", "K", "RR"])
+def test_models_custom_rates(Lbm, oracle, Q, model):
+    """Eq 11 / Eq 13-15 with a bulk rate and distinct third- and higher-order rates"""
+    g, o, fl = run_pair(Lbm, oracle, (7, 8, 9), Q, model, "SWAP_SOA", "f64", 21, kind="obstacle", omega=1.5,
+                        rates=(1.1, 1.3, 0.9))
+    assert pop_error(g, o, fl, Q, oracle, False) <= TOL64
+
+
+@pytest.mark.parametrize("scheme", ["2POP_SOA", "AA_SOA", "SWAP_AOS"])
+@pytest.mark.parametrize("model", ["BGK_W2", "TRT", "REG"])
+@pytest.mark.parametrize("Q", [19, 27])
+def test_fp32(Lbm, oracle, Q, model, scheme):
+    n = 16
+    omega = inputs.omega_from_re(n, 100)
+    g, o, fl = run_pair(Lbm, oracle, (n, n, n), Q, model, scheme, "f32", 100, omega=omega)
+    assert pop_error(g, o, fl, Q, oracle, True) <= TOL32
+
+
+def test_set_get_roundtrip_and_restart(Lbm, oracle):
+    """populations exported at an odd AA step and re-imported continue identically"""
+    shape = (9, 8, 10)
+    g, o, fl = run_pair(Lbm, oracle, shape, 19, "TRT", "AA_SOA", "f64", 5, kind="obstacle")
+    f5 = g.get_populations()
+    g2 = Lbm(*shape, lattice=19, collision="TRT", scheme="2POP_AOS", omega=1.7, dtype="f64")
+    fl2, uw = box_flags(*shape, "obstacle")
+    g2.set_flags(fl2, uw)
+    g2.set_populations(f5)
+    assert np.array_equal(g2.get_populations(), f5)
+    g.step(4)
+    g2.step(4)
+    o.step(4)
+    assert np.abs(g.get_populations() - g2.get_populations()).max() <= 1e-14
+    assert pop_error(g2, o, fl, 19, oracle, False) <= TOL64
+
+
+def test_state_errors(Lbm):
+    from paper_2010_11751_b200.binding import LbmError
+    g = Lbm(8, 8, 8)
+    with pytest.raises(LbmError):
+        g.step(1)
+    with pytest.raises(LbmError):
+        g.kinetic_energy()
+    with pytest.raises(LbmError):
+        Lbm(8, 8, 8, collision="K", dtype="f32")
+    with pytest.raises(LbmError):
+        Lbm(2, 8, 8)
+    assert g.kernel_launches >= 1 and g.device_bytes > 0
