@@ -75,6 +75,10 @@ int lbm_set_trt_magic(lbm_t* ctx, double lambda);
  * context dtype.  Resets the step count and the AA parity. */
 int lbm_init_equilibrium(lbm_t* ctx, const void* rho, const void* u);
 
+/* Same with rho [N] and u [3][N] already in DEVICE memory (context dtype, 16 B aligned);
+ * asynchronous on the stream; the buffers must stay valid until the stream reaches this point. */
+int lbm_init_equilibrium_device(lbm_t* ctx, const void* rho_dev, const void* u_dev);
+
 /* n collide-and-stream cycles (Eq 1-3) by the context's scheme; asynchronous on
  * the stream.  n >= 0. */
 int lbm_step(lbm_t* ctx, int n);
@@ -82,6 +86,9 @@ int lbm_step(lbm_t* ctx, int n);
 /* rho = sum_k f_k, u = sum_k c_k f_k / rho per cell of the pre-collision
  * populations at the current time; host outputs of the context dtype; synchronises. */
 int lbm_macroscopic(lbm_t* ctx, void* rho, void* u);
+
+/* Same into DEVICE buffers rho_dev [N], u_dev [3][N]; asynchronous on the stream. */
+int lbm_macroscopic_device(lbm_t* ctx, void* rho_dev, void* u_dev);
 
 /* E = sum over fluid cells of 1/2 rho |u|^2 (R19), accumulated in double with a fixed reduction
  * tree (bitwise repeatable); synchronises. */

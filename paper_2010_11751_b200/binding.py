@@ -24,7 +24,7 @@ FLUID, WALL, MOVING = 0, 1, 2
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = [
     "lbm_set_hooks", "lbm_create", "lbm_destroy", "lbm_set_flags", "lbm_set_relaxation", "lbm_set_trt_magic",
-    "lbm_init_equilibrium", "lbm_step", "lbm_macroscopic", "lbm_kinetic_energy", "lbm_get_populations",
+    "lbm_init_equilibrium", "lbm_init_equilibrium_device", "lbm_step", "lbm_macroscopic", "lbm_macroscopic_device", "lbm_kinetic_energy", "lbm_get_populations",
     "lbm_set_populations", "lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches",
     "lbm_sync", "lbm_set_variant", "lbm_last_error", "lbm_version",
 ]
@@ -59,6 +59,8 @@ def load_library(path=LIB_PATH):
     L.lbm_set_relaxation.argtypes = [vp, d, d, d]
     L.lbm_set_trt_magic.argtypes = [vp, d]
     L.lbm_init_equilibrium.argtypes = [vp, vp, vp]
+    L.lbm_init_equilibrium_device.argtypes = [vp, vp, vp]
+    L.lbm_macroscopic_device.argtypes = [vp, vp, vp]
     L.lbm_step.argtypes = [vp, i]
     L.lbm_macroscopic.argtypes = [vp, vp, vp]
     L.lbm_kinetic_energy.argtypes = [vp, dp]
@@ -177,6 +179,13 @@ class Lbm:
         u = np.empty((3, self.N), dtype=self.np_dtype) if out_u is None else out_u
         self._ck(self._L.lbm_macroscopic(self._h, _host_ptr(rho), _host_ptr(u)))
         return rho, u
+
+    def init_equilibrium_device(self, rho_ptr, u_ptr):
+        """rho_ptr, u_ptr: integer device addresses of [N] and [3][N] arrays of the context dtype."""
+        self._ck(self._L.lbm_init_equilibrium_device(self._h, C.c_void_p(int(rho_ptr)), C.c_void_p(int(u_ptr))))
+
+    def macroscopic_device(self, rho_ptr, u_ptr):
+        self._ck(self._L.lbm_macroscopic_device(self._h, C.c_void_p(int(rho_ptr)), C.c_void_p(int(u_ptr))))
 
     def kinetic_energy(self):
         e = C.c_double(0.0)

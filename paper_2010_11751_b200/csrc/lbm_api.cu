@@ -158,7 +158,8 @@ int load_mode(const lbm_ctx* c)
     return c->sto == STO_POST ? LD_PULL : c->sto == STO_AA_ODD ? LD_AAPULL : LD_LOCAL;
 }
 
-bool use_pull(const lbm_ctx* c) { return c->variant == V_GENERIC_PULL; }
+// the pull form is the default for 2-pop: aligned stores, measured faster on B200
+bool use_pull(const lbm_ctx* c) { return c->variant != V_GENERIC_PUSH; }
 
 // bring post-collision 2-pop storage back to canonical (one stream-only pass)
 int normalise(lbm_ctx* c)
@@ -310,6 +311,22 @@ int lbm_set_trt_magic(lbm_t* c, double lambda)
     return LBM_OK;
 }
 
+int lbm_init_equilibrium_device(lbm_t* c, const void* rho, const void* u)
+{
+    if (!c || !rho || !u) { set_err("null argument"); return LBM_E_ARG; }
+    const bool ext = !model_is_w2(c->model);
+    if (c->dtype == LBM_F64)
+        CK(aux_init_equilibrium<double>(c->Q, ext, c->soa, (double*)c->pop[0], c->code, c->g, (const double*)rho,
+                                        (const double*)u, c->stream));
+    else
+        CK(aux_init_equilibrium<float>(c->Q, ext, c->soa, (float*)c->pop[0], c->code, c->g, (const float*)rho,
+                                       (const float*)u, c->stream));
+    c->launches++;
+    c->sto = STO_CANON;
+    c->steps = 0;
+    return LBM_OK;
+}
+
 int lbm_init_equilibrium(lbm_t* c, const void* rho, const void* u)
 {
     if (!c || !rho || !u) { set_err("null argument"); return LBM_E_ARG; }
@@ -317,17 +334,8 @@ int lbm_init_equilibrium(lbm_t* c, const void* rho, const void* u)
     char* sc = (char*)c->scratch;
     CK(cudaMemcpyAsync(sc, rho, nb, cudaMemcpyHostToDevice, c->stream));
     CK(cudaMemcpyAsync(sc + nb, u, 3 * nb, cudaMemcpyHostToDevice, c->stream));
-    const bool ext = !model_is_w2(c->model);
-    if (c->dtype == LBM_F64)
-        CK(aux_init_equilibrium<double>(c->Q, ext, c->soa, (double*)c->pop[0], c->code, c->g, (const double*)sc,
-                                        (const double*)(sc + nb), c->stream));
-    else
-        CK(aux_init_equilibrium<float>(c->Q, ext, c->soa, (float*)c->pop[0], c->code, c->g, (const float*)sc,
-                                       (const float*)(sc + nb), c->stream));
-    c->launches++;
+    if (int rc = lbm_init_equilibrium_device(c, sc, sc + nb)) return rc;
     CK(cudaStreamSynchronize(c->stream));  // host buffers are only read during the call
-    c->sto = STO_CANON;
-    c->steps = 0;
     return LBM_OK;
 }
 
@@ -370,19 +378,26 @@ int lbm_step(lbm_t* c, int n)
     return LBM_OK;
 }
 
-int lbm_macroscopic(lbm_t* c, void* rho, void* u)
+int lbm_macroscopic_device(lbm_t* c, void* rho, void* u)
 {
     if (!c || !rho || !u) { set_err("null argument"); return LBM_E_ARG; }
     if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
+    if (c->dtype == LBM_F64)
+        CK(aux_macroscopic<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr), (double*)rho,
+                                   (double*)u, c->stream));
+    else
+        CK(aux_macroscopic<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr), (float*)rho,
+                                  (float*)u, c->stream));
+    c->launches++;
+    return LBM_OK;
+}
+
+int lbm_macroscopic(lbm_t* c, void* rho, void* u)
+{
+    if (!c || !rho || !u) { set_err("null argument"); return LBM_E_ARG; }
     const size_t nb = (size_t)c->g.n * c->elem;
     char* sc = (char*)c->scratch;
-    if (c->dtype == LBM_F64)
-        CK(aux_macroscopic<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr), (double*)sc,
-                                   (double*)(sc + nb), c->stream));
-    else
-        CK(aux_macroscopic<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr), (float*)sc,
-                                  (float*)(sc + nb), c->stream));
-    c->launches++;
+    if (int rc = lbm_macroscopic_device(c, sc, sc + nb)) return rc;
     CK(cudaMemcpyAsync(rho, sc, nb, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaMemcpyAsync(u, sc + nb, 3 * nb, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
@@ -470,7 +485,7 @@ int lbm_set_variant(lbm_t* c, int variant)
 {
     if (!c) { set_err("null context"); return LBM_E_ARG; }
     if (variant < 0 || variant >= V_COUNT) { set_err("unknown variant %d", variant); return LBM_E_ARG; }
-    if (c->fam == FAM_2POP && variant != V_GENERIC_PULL) {
+    if (c->fam == FAM_2POP && variant == V_GENERIC_PUSH) {
         if (int rc = normalise(c)) return rc;
     }
     c->variant = variant;

@@ -1,0 +1,62 @@
+"""Host logic of bench.py: roofline arithmetic, the replicas aggregation under gloo (world size 2), the reference arm."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_bytes_per_update():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.bytes_per_update(19, "f64", "2POP_SOA") == 304     # 2*19*8, Eq 16
+    assert bench.bytes_per_update(19, "f32", "AA_SOA") == 152
+    assert bench.bytes_per_update(19, "f64", "SWAP_SOA") == 592
+    assert bench.bytes_per_update(27, "f64", "SWAP_AOS") == 848
+    assert bench.bytes_per_update(27, "f64", "AA_AOS") == 432
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, %r)
+import torch.distributed as dist
+import bench
+dist.init_process_group(backend="gloo")
+r = dist.get_rank()
+ms, units = bench.aggregate(dist, 10.0 + 5.0 * r, 1000 * (r + 1))
+dist.barrier()
+assert ms == 15.0 and units == 3000.0, (ms, units)
+print("OK", r)
+dist.destroy_process_group()
+"""
+
+
+def test_aggregate_gloo_world2(tmp_path):
+    script = tmp_path / "w.py"
+    script.write_text(_WORKER % ROOT)
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+           "--master-addr", "127.0.0.1", "--master-port", "29517", str(script)]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=300)
+    assert r.returncode == 0, r.stdout + r.stderr
+    assert r.stdout.count("OK") == 2
+
+
+def test_reference_arm_prints_one_json_line():
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "1",
+                        "--steps", "3", "--warmup", "1"], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr
+    lines = [l for l in r.stdout.splitlines() if l.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["metric"] == "MLUPS" and d["value"] > 0
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_reference_arm_other_ranks_exit_quietly():
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "1",
+                        "--steps", "2", "--warmup", "1"], capture_output=True, text=True, timeout=600, env=env)
+    assert r.returncode == 0 and r.stdout.strip() == ""
