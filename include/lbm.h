@@ -96,6 +96,10 @@ int lbm_kinetic_energy(lbm_t* ctx, double* e);
 
 /* Pre-collision populations at the current time, canonical [Q][N] order, context dtype, host. */
 int lbm_get_populations(lbm_t* ctx, void* f);
+/* The same for m listed cells only: cells = host int32 [m] of cell indices in [0, N), f = host
+ * [Q][m] of the context dtype (f[k*m + t] = f_k(cells[t])).  Lets the parity tests sample a
+ * 512^3 lattice without a 20 GB export.  0 <= m <= N. */
+int lbm_get_populations_at(lbm_t* ctx, const int32_t* cells, int m, void* f);
 /* Load populations (same format); resets the AA parity to even. */
 int lbm_set_populations(lbm_t* ctx, const void* f);
 
@@ -110,6 +114,10 @@ int lbm_sync(lbm_t* ctx);
 /* Select an implementation variant of the step kernels (0 = default); used by the bench sweep.
  * Unknown variants return LBM_E_ARG.  Results are identical across variants. */
 int lbm_set_variant(lbm_t* ctx, int variant);
+
+/* Threads per block of the step kernels (tuning knob of the sweep; multiple of 32 in [32, 256];
+ * default 128).  Results do not depend on it. */
+int lbm_set_block(lbm_t* ctx, int threads);
 
 const char* lbm_last_error(void);
 const char* lbm_version(void);

@@ -24,9 +24,9 @@ FLUID, WALL, MOVING = 0, 1, 2
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = [
     "lbm_set_hooks", "lbm_create", "lbm_destroy", "lbm_set_flags", "lbm_set_relaxation", "lbm_set_trt_magic",
-    "lbm_init_equilibrium", "lbm_init_equilibrium_device", "lbm_step", "lbm_macroscopic", "lbm_macroscopic_device", "lbm_kinetic_energy", "lbm_get_populations",
+    "lbm_init_equilibrium", "lbm_init_equilibrium_device", "lbm_step", "lbm_macroscopic", "lbm_macroscopic_device", "lbm_kinetic_energy", "lbm_get_populations", "lbm_get_populations_at",
     "lbm_set_populations", "lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches",
-    "lbm_sync", "lbm_set_variant", "lbm_last_error", "lbm_version",
+    "lbm_sync", "lbm_set_variant", "lbm_set_block", "lbm_last_error", "lbm_version",
 ]
 
 
@@ -65,12 +65,14 @@ def load_library(path=LIB_PATH):
     L.lbm_macroscopic.argtypes = [vp, vp, vp]
     L.lbm_kinetic_energy.argtypes = [vp, dp]
     L.lbm_get_populations.argtypes = [vp, vp]
+    L.lbm_get_populations_at.argtypes = [vp, vp, i, vp]
     L.lbm_set_populations.argtypes = [vp, vp]
     for name in ("lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches"):
         getattr(L, name).restype = C.c_longlong
         getattr(L, name).argtypes = [vp]
     L.lbm_sync.argtypes = [vp]
     L.lbm_set_variant.argtypes = [vp, i]
+    L.lbm_set_block.argtypes = [vp, i]
     L.lbm_last_error.restype = C.c_char_p
     L.lbm_version.restype = C.c_char_p
     _lib = L
@@ -164,6 +166,9 @@ class Lbm:
     def set_variant(self, variant):
         self._ck(self._L.lbm_set_variant(self._h, VARIANTS[variant] if isinstance(variant, str) else int(variant)))
 
+    def set_block(self, threads):
+        self._ck(self._L.lbm_set_block(self._h, int(threads)))
+
     def init_equilibrium(self, rho, u):
         r, uu = self._arr(rho, self.N), self._arr(u, 3 * self.N)
         self._ck(self._L.lbm_init_equilibrium(self._h, _host_ptr(r), _host_ptr(uu)))
@@ -195,6 +200,13 @@ class Lbm:
     def get_populations(self):
         f = np.empty((self.Q, self.N), dtype=self.np_dtype)
         self._ck(self._L.lbm_get_populations(self._h, _host_ptr(f)))
+        return f
+
+    def get_populations_at(self, cells):
+        """f[Q, m] of the listed cell indices (int32)."""
+        cc = np.ascontiguousarray(cells, dtype=np.int32).reshape(-1)
+        f = np.empty((self.Q, cc.size), dtype=self.np_dtype)
+        self._ck(self._L.lbm_get_populations_at(self._h, _host_ptr(cc), int(cc.size), _host_ptr(f)))
         return f
 
     def set_populations(self, f):

@@ -5,23 +5,37 @@
 
 namespace lbm {
 
-// cell code from raw flags: fluid cells on the box faces (periodic seam) or next to a non-fluid
-// cell get CODE_EDGE.  The 27-neighbourhood is used for both lattices (a superset for D3Q19).
-__global__ void classify_kernel(const uint8_t* __restrict__ flags, uint8_t* __restrict__ code, Geo g)
+// cell code and link mask (kernels.cuh) from raw flags.  A fluid cell gets CODE_EDGE when its
+// mask is non-zero: a link of the lattice ends on a non-fluid cell, or the cell lies on a face of
+// the box (periodic seam).
+template <int Q>
+__global__ void classify_kernel(const uint8_t* __restrict__ flags, uint8_t* __restrict__ code,
+                                unsigned long long* __restrict__ mask, Geo g)
 {
+    using L = Lat<Q>;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.n) return;
     const uint8_t fl = flags[i];
-    if (fl != 0) { code[i] = fl == 2 ? CODE_MOVING : CODE_WALL; return; }
+    if (fl != 0) { code[i] = fl == 2 ? CODE_MOVING : CODE_WALL; mask[i] = 0ull; return; }
     const int z = i % g.nz, y = (i / g.nz) % g.ny, x = i / (g.nz * g.ny);
-    bool edge = x == 0 || y == 0 || z == 0 || x == g.nx - 1 || y == g.ny - 1 || z == g.nz - 1;
-    if (!edge) {
-        for (int dx = -1; dx <= 1; ++dx)
-            for (int dy = -1; dy <= 1; ++dy)
-                for (int dz = -1; dz <= 1; ++dz)
-                    edge |= flags[((x + dx) * g.ny + (y + dy)) * g.nz + (z + dz)] != 0;
-    }
-    code[i] = edge ? CODE_EDGE : CODE_BULK;
+    unsigned long long m = 0ull;
+    if (x == 0) m |= 1ull << (MASK_FACE_SHIFT + 0);
+    if (x == g.nx - 1) m |= 1ull << (MASK_FACE_SHIFT + 1);
+    if (y == 0) m |= 1ull << (MASK_FACE_SHIFT + 2);
+    if (y == g.ny - 1) m |= 1ull << (MASK_FACE_SHIFT + 3);
+    if (z == 0) m |= 1ull << (MASK_FACE_SHIFT + 4);
+    if (z == g.nz - 1) m |= 1ull << (MASK_FACE_SHIFT + 5);
+    static_for<Q>([&](auto kc) {
+        constexpr int k = kc;
+        if constexpr (k != L::REST) {
+            const int n = (wrap1(x + L::cx(k), g.nx) * g.ny + wrap1(y + L::cy(k), g.ny)) * g.nz + wrap1(z + L::cz(k), g.nz);
+            const uint8_t nf = flags[n];
+            if (nf != 0) m |= 1ull << link_of<Q>(k);
+            if (nf == 2) m |= 1ull << (MASK_MOVING_SHIFT + link_of<Q>(k));
+        }
+    });
+    code[i] = m ? CODE_EDGE : CODE_BULK;
+    mask[i] = m;
 }
 
 // energy stage 2: one block sums the per-block partials in a fixed order
@@ -47,19 +61,20 @@ template <class T, int Q, bool SOA>
 __global__ void __launch_bounds__(256) stream_only_kernel(const StepArgs<T> a)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= a.g.n) return;
-    const uint8_t mycode = a.code[i];
-    if (mycode & 3) return;
+    const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
+    if (!cs.active) return;
     T f[Q];
-    load_cell<T, Q, SOA, LD_PULL>(a.src, a.code, a.g, a.wterm, i, mycode, f);
-    store_cell<T, Q, SOA, ST_LOCAL>(a.dst, a.code, a.g, a.wterm, i, mycode, f);
+    load_cell<T, Q, SOA, LD_PULL>(a.src, a.g, a.wterm, i, cs.masked, cs.mask, f);
+    store_cell<T, Q, SOA, ST_LOCAL>(a.dst, a.g, a.wterm, i, cs.masked, cs.mask, f);
 }
 
 static inline int blocks_for(int n, int block) { return (n + block - 1) / block; }
 
-cudaError_t aux_classify(const uint8_t* flags, uint8_t* code, const Geo& g, cudaStream_t s)
+cudaError_t aux_classify(int Q, const uint8_t* flags, uint8_t* code, unsigned long long* mask, const Geo& g, cudaStream_t s)
 {
-    classify_kernel<<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, g);
+    if (Q == 19) classify_kernel<19><<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, mask, g);
+    else if (Q == 27) classify_kernel<27><<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, mask, g);
+    else return cudaErrorInvalidValue;
     return cudaGetLastError();
 }
 
@@ -123,10 +138,10 @@ cudaError_t aux_energy(int Q, bool soa, int load, const StepArgs<T>& a, double* 
 
 template <class T>
 cudaError_t aux_extract_plane(int Q, bool soa, const T* pop, const uint8_t* code, const Geo& g, const PlaneArgs& p,
-                              T* out, cudaStream_t s)
+                              T* out, const int* cells, int m, cudaStream_t s)
 {
-    const int grid = blocks_for(g.n, 256);
-#define CALL(QQ, SS) extract_plane_kernel<T, QQ, SS><<<grid, 256, 0, s>>>(pop, code, g, p, out)
+    const int grid = blocks_for(m, 256);
+#define CALL(QQ, SS) extract_plane_kernel<T, QQ, SS><<<grid, 256, 0, s>>>(pop, code, g, p, out, cells, m)
     LBM_QS_DISPATCH(Q, soa, CALL);
 #undef CALL
     return cudaGetLastError();
@@ -169,7 +184,7 @@ cudaError_t aux_stream_only(int Q, bool soa, const StepArgs<T>& a, cudaStream_t 
     template cudaError_t aux_macroscopic<T>(int, bool, int, const StepArgs<T>&, T*, T*, cudaStream_t);                  \
     template cudaError_t aux_energy<T>(int, bool, int, const StepArgs<T>&, double*, int, double*, cudaStream_t);        \
     template cudaError_t aux_extract_plane<T>(int, bool, const T*, const uint8_t*, const Geo&, const PlaneArgs&, T*,    \
-                                              cudaStream_t);                                                            \
+                                              const int*, int, cudaStream_t);                                                           \
     template cudaError_t aux_insert_plane<T>(int, bool, T*, const uint8_t*, const Geo&, int, double, const T*,          \
                                              cudaStream_t);                                                             \
     template cudaError_t aux_swap_stream<T>(int, bool, const StepArgs<T>&, cudaStream_t);                               \

@@ -29,7 +29,7 @@ template <class T, int Q, int MODEL>
 cudaError_t launch_step(int kind, bool soa, int block, const StepArgs<T>& a, cudaStream_t s);
 
 // defined in aux.cu
-cudaError_t aux_classify(const uint8_t* flags, uint8_t* code, const Geo& g, cudaStream_t s);
+cudaError_t aux_classify(int Q, const uint8_t* flags, uint8_t* code, unsigned long long* mask, const Geo& g, cudaStream_t s);
 template <class T>
 cudaError_t aux_init_equilibrium(int Q, bool ext, bool soa, T* pop, const uint8_t* code, const Geo& g, const T* rho,
                                  const T* u, cudaStream_t s);
@@ -40,7 +40,7 @@ cudaError_t aux_energy(int Q, bool soa, int load, const StepArgs<T>& a, double* 
                        cudaStream_t s);
 template <class T>
 cudaError_t aux_extract_plane(int Q, bool soa, const T* pop, const uint8_t* code, const Geo& g, const PlaneArgs& p,
-                              T* out, cudaStream_t s);
+                              T* out, const int* cells, int m, cudaStream_t s);
 template <class T>
 cudaError_t aux_insert_plane(int Q, bool soa, T* pop, const uint8_t* code, const Geo& g, int k, double weight,
                              const T* in, cudaStream_t s);

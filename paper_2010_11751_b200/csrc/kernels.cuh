@@ -10,10 +10,18 @@
 //
 // with w_k = -6 t_k rho_w c_k.u_w (Eq 3; rho_w = 1, L92; zero for a resting wall).
 // Instead of the paper's wall cells that store w_k in their 19 slots (Eq 4-5) a byte per
-// cell says what the cell is; only fluid cells that touch a wall or the periodic seam take the
-// slow path that looks at neighbour bytes, all others use fixed offsets.
+// cell says what the cell is, and fluid cells that touch a non-fluid cell or a face of the box
+// carry a 64-bit link mask (built once by classify_kernel):
 //
-// cell code byte: 0 = bulk fluid, 1 = wall, 2 = moving wall, 4 = fluid that needs the slow path.
+//   bits  0..25  link l: the neighbour at x + c_k is not fluid            (l = k, rest skipped)
+//   bits 26..51  link l: that neighbour is a MOVING wall
+//   bits 52..57  the cell lies on the face x=0, x=nx-1, y=0, y=ny-1, z=0, z=nz-1 (periodic seam)
+//
+// A warp in which no lane has a mask runs the pure path (fixed offsets, no tests); a warp with at
+// least one masked lane runs the masked path for all its lanes (selects on mask bits, no
+// divergence, no integer division).  Both give the same values for bulk cells.
+//
+// cell code byte: 0 = bulk fluid, 1 = wall, 2 = moving wall, 4 = fluid with a non-zero link mask.
 #pragma once
 #include "collision.cuh"
 
@@ -22,6 +30,7 @@ namespace lbm {
 enum { LD_LOCAL = 0, LD_PULL, LD_AAPULL };
 enum { ST_LOCAL = 0, ST_SWAPPED, ST_PUSH };
 enum { CODE_BULK = 0, CODE_WALL = 1, CODE_MOVING = 2, CODE_EDGE = 4 };
+enum { MASK_MOVING_SHIFT = 26, MASK_FACE_SHIFT = 52 };
 
 struct Geo {
     int nx, ny, nz;
@@ -34,6 +43,7 @@ struct StepArgs {
     const T* src;
     T* dst;
     const uint8_t* code;
+    const unsigned long long* mask;
     Geo g;
     Rates<T> rt;
     T wterm[27];  // w_k
@@ -47,17 +57,6 @@ __device__ __forceinline__ long long slot(const Geo& g, int k, long long i)
 
 __device__ __forceinline__ int wrap1(int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); }
 
-// index of the cell at (x + sx*cx, y + sy*cy, z + sz*cz) with periodic wrap
-template <int Q, int K, int SIGN>
-__device__ __forceinline__ int neighbour(const Geo& g, int x, int y, int z)
-{
-    using L = Lat<Q>;
-    const int xx = wrap1(x + SIGN * L::cx(K), g.nx);
-    const int yy = wrap1(y + SIGN * L::cy(K), g.ny);
-    const int zz = wrap1(z + SIGN * L::cz(K), g.nz);
-    return (xx * g.ny + yy) * g.nz + zz;
-}
-
 template <int Q, int K>
 __device__ __forceinline__ int offset(const Geo& g)
 {
@@ -65,64 +64,129 @@ __device__ __forceinline__ int offset(const Geo& g)
     return (L::cx(K) * g.ny + L::cy(K)) * g.nz + L::cz(K);
 }
 
+// link index of direction k in the mask (the rest velocity has no link)
+template <int Q>
+__host__ __device__ constexpr int link_of(int k) { return k < Lat<Q>::REST ? k : k - 1; }
+
+// per-thread view of a link mask: wrapped index offsets to the six axis neighbours
+struct Edge {
+    unsigned long long m;
+    int oxm, oxp, oym, oyp, ozm, ozp;
+    __device__ __forceinline__ Edge(unsigned long long mask, const Geo& g) : m(mask)
+    {
+        const int sx = g.ny * g.nz, sy = g.nz;
+        const unsigned f = (unsigned)(mask >> MASK_FACE_SHIFT);
+        oxm = (f & 1u) ? (g.nx - 1) * sx : -sx;
+        oxp = (f & 2u) ? -(g.nx - 1) * sx : sx;
+        oym = (f & 4u) ? (g.ny - 1) * sy : -sy;
+        oyp = (f & 8u) ? -(g.ny - 1) * sy : sy;
+        ozm = (f & 16u) ? (g.nz - 1) : -1;
+        ozp = (f & 32u) ? -(g.nz - 1) : 1;
+    }
+    // index offset to the cell at x + SIGN * c_K, periodic wrap included
+    template <int Q, int K, int SIGN>
+    __device__ __forceinline__ int off() const
+    {
+        using L = Lat<Q>;
+        constexpr int dx = SIGN * L::cx(K), dy = SIGN * L::cy(K), dz = SIGN * L::cz(K);
+        int o = 0;
+        if constexpr (dx == 1) o += oxp;
+        if constexpr (dx == -1) o += oxm;
+        if constexpr (dy == 1) o += oyp;
+        if constexpr (dy == -1) o += oym;
+        if constexpr (dz == 1) o += ozp;
+        if constexpr (dz == -1) o += ozm;
+        return o;
+    }
+    template <int Q, int K>
+    __device__ __forceinline__ bool solid() const { return (m >> link_of<Q>(K)) & 1ull; }
+    template <int Q, int K>
+    __device__ __forceinline__ bool moving() const { return (m >> (MASK_MOVING_SHIFT + link_of<Q>(K))) & 1ull; }
+};
+
 // ------------------------------------------------------------------ load / store of one cell
+// `masked` must be warp-uniform; mask is this cell's link mask (0 for a bulk cell)
 template <class T, int Q, bool SOA, int LOAD>
-__device__ __forceinline__ void load_cell(const T* __restrict__ src, const uint8_t* __restrict__ code, const Geo& g,
-                                          const T (&wterm)[27], int i, uint8_t mycode, T (&f)[Q])
+__device__ __forceinline__ void load_cell(const T* __restrict__ src, const Geo& g, const T (&wterm)[27], int i,
+                                          bool masked, unsigned long long mask, T (&f)[Q])
 {
     using L = Lat<Q>;
     if (LOAD == LD_LOCAL) {
         static_for<Q>([&](auto kc) { f[kc] = src[slot<SOA, Q>(g, kc, i)]; });
-    } else if (mycode == CODE_BULK) {
+    } else if (!masked) {
         static_for<Q>([&](auto kc) {
             constexpr int k = kc;
             constexpr int s = LOAD == LD_PULL ? k : L::opp(k);
             f[k] = src[slot<SOA, Q>(g, s, (long long)i - offset<Q, k>(g))];
         });
     } else {
-        const int z = i % g.nz, y = (i / g.nz) % g.ny, x = i / (g.nz * g.ny);
+        const Edge e(mask, g);
         static_for<Q>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
             if constexpr (k == L::REST) {
                 f[k] = src[slot<SOA, Q>(g, k, i)];
             } else {
-                const int n = neighbour<Q, k, -1>(g, x, y, z);
-                const int nc = code[n] & 3;
-                if (nc == 0) f[k] = src[slot<SOA, Q>(g, LOAD == LD_PULL ? k : kb, n)];
-                else f[k] = src[slot<SOA, Q>(g, LOAD == LD_PULL ? kb : k, i)] + (nc == CODE_MOVING ? wterm[kb] : T(0));
+                // the upstream neighbour x - c_k = x + c_kbar
+                constexpr int s_fluid = LOAD == LD_PULL ? k : kb, s_wall = LOAD == LD_PULL ? kb : k;
+                const bool sol = e.template solid<Q, kb>();
+                const long long a_fluid = slot<SOA, Q>(g, s_fluid, (long long)i + e.template off<Q, k, -1>());
+                const long long a_wall = slot<SOA, Q>(g, s_wall, i);
+                T v = src[sol ? a_wall : a_fluid];
+                if (e.template moving<Q, kb>()) v += wterm[kb];
+                f[k] = v;
             }
         });
     }
 }
 
 template <class T, int Q, bool SOA, int STORE>
-__device__ __forceinline__ void store_cell(T* __restrict__ dst, const uint8_t* __restrict__ code, const Geo& g,
-                                           const T (&wterm)[27], int i, uint8_t mycode, const T (&f)[Q])
+__device__ __forceinline__ void store_cell(T* __restrict__ dst, const Geo& g, const T (&wterm)[27], int i, bool masked,
+                                           unsigned long long mask, const T (&f)[Q])
 {
     using L = Lat<Q>;
     if (STORE == ST_LOCAL) {
         static_for<Q>([&](auto kc) { dst[slot<SOA, Q>(g, kc, i)] = f[kc]; });
     } else if (STORE == ST_SWAPPED) {
         static_for<Q>([&](auto kc) { dst[slot<SOA, Q>(g, L::opp(kc), i)] = f[kc]; });
-    } else if (mycode == CODE_BULK) {
+    } else if (!masked) {
         static_for<Q>([&](auto kc) {
             constexpr int k = kc;
             dst[slot<SOA, Q>(g, k, (long long)i + offset<Q, k>(g))] = f[k];
         });
     } else {
-        const int z = i % g.nz, y = (i / g.nz) % g.ny, x = i / (g.nz * g.ny);
+        const Edge e(mask, g);
         static_for<Q>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
             if constexpr (k == L::REST) {
                 dst[slot<SOA, Q>(g, k, i)] = f[k];
             } else {
-                const int n = neighbour<Q, k, +1>(g, x, y, z);
-                const int nc = code[n] & 3;
-                if (nc == 0) dst[slot<SOA, Q>(g, k, n)] = f[k];
-                else dst[slot<SOA, Q>(g, kb, i)] = f[k] + (nc == CODE_MOVING ? wterm[k] : T(0));
+                const bool sol = e.template solid<Q, k>();
+                const long long a_fluid = slot<SOA, Q>(g, k, (long long)i + e.template off<Q, k, +1>());
+                const long long a_wall = slot<SOA, Q>(g, kb, i);
+                T v = f[k];
+                if (e.template moving<Q, k>()) v += wterm[k];
+                dst[sol ? a_wall : a_fluid] = v;
             }
         });
     }
+}
+
+// what every cell kernel starts with: is this thread's cell fluid, and does its warp need masks
+struct CellState {
+    bool active, masked;
+    unsigned long long mask;
+};
+__device__ __forceinline__ CellState cell_state(const uint8_t* __restrict__ code,
+                                                const unsigned long long* __restrict__ mask, long long i, int n)
+{
+    CellState s;
+    uint8_t c = CODE_WALL;
+    if (i < n) c = code[i];
+    s.active = !(c & 3);
+    const bool edge = c == CODE_EDGE;
+    s.masked = __any_sync(0xffffffffu, edge);
+    s.mask = edge ? mask[i] : 0ull;
+    return s;
 }
 
 // ------------------------------------------------------------------ the fused step
@@ -131,56 +195,69 @@ __global__ void __launch_bounds__(256) step_kernel(const StepArgs<T> a)
 {
     constexpr bool SHIFT = sizeof(T) == 4;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= a.g.n) return;
-    const uint8_t mycode = a.code[i];
-    if (mycode & 3) return;  // solid cells hold no populations
+    const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
+    if (!cs.active) return;  // solid cells hold no populations
     T f[Q];
-    load_cell<T, Q, SOA, LOAD>(a.src, a.code, a.g, a.wterm, i, mycode, f);
+    load_cell<T, Q, SOA, LOAD>(a.src, a.g, a.wterm, i, cs.masked, cs.mask, f);
     collide<Q, MODEL, SHIFT>(f, a.rt);
-    store_cell<T, Q, SOA, STORE>(a.dst, a.code, a.g, a.wterm, i, mycode, f);
+    store_cell<T, Q, SOA, STORE>(a.dst, a.g, a.wterm, i, cs.masked, cs.mask, f);
 }
 
 // ------------------------------------------------------------------ swap scheme, pass 2
 // After pass 1 pop_kbar(x) holds f_out_k(x).  For the half set k < NH (R5): exchange pop_kbar(x)
 // with pop_k(x + c_k) when that neighbour is fluid, else add w_k in place (the value already sits
 // in the slot Eq 3 sends it to); and when the neighbour at x - c_k is a wall, add w_kbar to pop_k(x).
-// Every slot is touched by exactly one thread (Table 1).
+// Every slot is touched by exactly one thread (Table 1), so all loads
+// are issued before the first store.
 template <class T, int Q, bool SOA>
 __global__ void __launch_bounds__(256) swap_stream_kernel(const StepArgs<T> a)
 {
     using L = Lat<Q>;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= a.g.n) return;
-    const uint8_t mycode = a.code[i];
-    if (mycode & 3) return;
+    const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
+    if (!cs.active) return;
     T* __restrict__ pop = a.dst;
     const Geo& g = a.g;
-    if (mycode == CODE_BULK) {
+    T va[L::NH], vb[L::NH];
+    if (!cs.masked) {
         static_for<L::NH>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
-            const long long pa = slot<SOA, Q>(g, kb, i);
-            const long long pb = slot<SOA, Q>(g, k, (long long)i + offset<Q, k>(g));
-            const T va = pop[pa], vb = pop[pb];
-            pop[pa] = vb;
-            pop[pb] = va;
+            va[k] = pop[slot<SOA, Q>(g, kb, i)];
+            vb[k] = pop[slot<SOA, Q>(g, k, (long long)i + offset<Q, k>(g))];
+        });
+        static_for<L::NH>([&](auto kc) {
+            constexpr int k = kc, kb = L::opp(k);
+            pop[slot<SOA, Q>(g, kb, i)] = vb[k];
+            pop[slot<SOA, Q>(g, k, (long long)i + offset<Q, k>(g))] = va[k];
         });
     } else {
-        const int z = i % g.nz, y = (i / g.nz) % g.ny, x = i / (g.nz * g.ny);
+        // a link to a solid neighbour exchanges nothing: slot kbar of this cell keeps its value
+        // (plus w_k), and slot k of this cell is read and rewritten with w_kbar added when the
+        // neighbour at x - c_k is a moving wall
+        const Edge e(cs.mask, g);
         static_for<L::NH>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
-            const int n = neighbour<Q, k, +1>(g, x, y, z);
-            const int nc = a.code[n] & 3;
+            const bool sol = e.template solid<Q, k>();
+            const long long pb = sol ? slot<SOA, Q>(g, k, i) : slot<SOA, Q>(g, k, (long long)i + e.template off<Q, k, +1>());
+            va[k] = pop[slot<SOA, Q>(g, kb, i)];
+            vb[k] = pop[pb];
+        });
+        static_for<L::NH>([&](auto kc) {
+            constexpr int k = kc, kb = L::opp(k);
+            const bool sol = e.template solid<Q, k>();
+            const bool back_moving = e.template moving<Q, kb>();   // neighbour at x - c_k
             const long long pa = slot<SOA, Q>(g, kb, i);
-            if (nc == 0) {
-                const long long pb = slot<SOA, Q>(g, k, n);
-                const T va = pop[pa], vb = pop[pb];
-                pop[pa] = vb;
-                pop[pb] = va;
-            } else if (nc == CODE_MOVING) {
-                pop[pa] += a.wterm[k];
+            if (!sol) {
+                const long long pb = slot<SOA, Q>(g, k, (long long)i + e.template off<Q, k, +1>());
+                pop[pa] = vb[k];
+                pop[pb] = va[k];
+                // pop_k(x) belongs to the exchange of the cell at x - c_k unless that one is solid
+                if (back_moving) pop[slot<SOA, Q>(g, k, i)] += a.wterm[kb];
+            } else {
+                // vb[k] holds pop_k(x) here
+                if (e.template moving<Q, k>()) pop[pa] = va[k] + a.wterm[k];
+                if (back_moving) pop[slot<SOA, Q>(g, k, i)] = vb[k] + a.wterm[kb];
             }
-            const int m = neighbour<Q, k, -1>(g, x, y, z);
-            if ((a.code[m] & 3) == CODE_MOVING) pop[slot<SOA, Q>(g, k, i)] += a.wterm[kb];
         });
     }
 }
@@ -213,12 +290,12 @@ __global__ void macroscopic_kernel(const T* __restrict__ pop, const uint8_t* __r
 {
     constexpr bool SHIFT = sizeof(T) == 4;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const CellState cs = cell_state(code, a.mask, i, g.n);
     if (i >= g.n) return;
-    const uint8_t mycode = code[i];
     T r = T(0), uu[3] = {T(0), T(0), T(0)};
-    if (!(mycode & 3)) {
+    if (cs.active) {
         T f[Q], dr;
-        load_cell<T, Q, SOA, LOAD>(pop, code, g, a.wterm, i, mycode, f);
+        load_cell<T, Q, SOA, LOAD>(pop, g, a.wterm, i, cs.masked, cs.mask, f);
         moments_rho_u<Q, SHIFT>(f, r, dr, uu);
     }
     rho[i] = r;
@@ -234,11 +311,13 @@ __global__ void __launch_bounds__(256) energy_kernel(const T* __restrict__ pop, 
 {
     constexpr bool SHIFT = sizeof(T) == 4;
     double e = 0.0;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < g.n; i += (long long)gridDim.x * blockDim.x) {
-        const uint8_t mycode = code[i];
-        if (mycode & 3) continue;
+    // the trip count is the same for every lane of a warp (cell_state votes across the warp)
+    const long long n32 = ((long long)g.n + 31) & ~31LL;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n32; i += (long long)gridDim.x * blockDim.x) {
+        const CellState cs = cell_state(code, a.mask, i, g.n);
+        if (!cs.active) continue;
         T f[Q], r, dr, uu[3];
-        load_cell<T, Q, SOA, LOAD>(pop, code, g, a.wterm, (int)i, mycode, f);
+        load_cell<T, Q, SOA, LOAD>(pop, g, a.wterm, (int)i, cs.masked, cs.mask, f);
         moments_rho_u<Q, SHIFT>(f, r, dr, uu);
         e += 0.5 * (double)r * ((double)uu[0] * uu[0] + (double)uu[1] * uu[1] + (double)uu[2] * uu[2]);
     }
@@ -264,13 +343,15 @@ struct PlaneArgs {
     double wterm;   // w_kbar
     double weight;  // t_k, added back when the storage is shifted
 };
+// cells == nullptr: the whole plane (out[i], i < n); else a gather of m listed cells (out[t] = f_k(cells[t]))
 template <class T, int Q, bool SOA>
 __global__ void extract_plane_kernel(const T* __restrict__ pop, const uint8_t* __restrict__ code, Geo g, PlaneArgs p,
-                                     T* __restrict__ out)
+                                     T* __restrict__ out, const int* __restrict__ cells, int m)
 {
     constexpr bool SHIFT = sizeof(T) == 4;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= g.n) return;
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= m) return;
+    const int i = cells ? cells[t] : t;
     T v = T(0);
     if (!(code[i] & 3)) {
         int n = i;
@@ -283,7 +364,7 @@ __global__ void extract_plane_kernel(const T* __restrict__ pop, const uint8_t* _
         else v = pop[slot<SOA, Q>(g, p.slot_wall, i)] + (nc == CODE_MOVING ? T(p.wterm) : T(0));
         if (SHIFT) v += T(p.weight);
     }
-    out[i] = v;
+    out[t] = v;
 }
 template <class T, int Q, bool SOA>
 __global__ void insert_plane_kernel(T* __restrict__ pop, const uint8_t* __restrict__ code, Geo g, int k, double weight,

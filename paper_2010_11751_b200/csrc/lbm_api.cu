@@ -49,6 +49,7 @@ struct lbm_ctx {
     size_t pop_elems;   // elements in one population array
     void* pop[2];       // [1] only for FAM_2POP
     uint8_t* code;
+    unsigned long long* mask;  // link masks (kernels.cuh), [N]
     void* scratch;      // 4 planes of N elements (rho,u staging; plane import/export)
     double* partial;    // energy partial sums
     double* e_dev;
@@ -99,6 +100,7 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst)
     a.src = (const T*)src;
     a.dst = (T*)dst;
     a.code = c->code;
+    a.mask = c->mask;
     a.g = c->g;
     a.rt.omega = (T)c->omega;
     a.rt.omega_bulk = (T)c->omega_bulk;
@@ -241,6 +243,7 @@ lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme
     }
     if (ok) { c->code = (uint8_t*)dev_alloc(c, (size_t)c->g.n); ok = c->code != nullptr; }
     if (ok) ok = cudaMemsetAsync(c->code, 0, (size_t)c->g.n, c->stream) == cudaSuccess;
+    if (ok) { c->mask = (unsigned long long*)dev_alloc(c, sizeof(unsigned long long) * (size_t)c->g.n); ok = c->mask != nullptr; }
     if (ok) { c->scratch = dev_alloc(c, 4 * (size_t)c->g.n * c->elem); ok = c->scratch != nullptr; }
     c->n_partial = 148 * 8;
     if (ok) { c->partial = (double*)dev_alloc(c, sizeof(double) * (c->n_partial + 1)); ok = c->partial != nullptr; }
@@ -253,7 +256,7 @@ lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme
     // cells on the faces of a fully periodic box still need the wrap: classify with all-fluid flags
     // (scratch is large enough to stand in for a zero flag array of N bytes)
     if (cudaMemsetAsync(c->scratch, 0, (size_t)c->g.n, c->stream) != cudaSuccess ||
-        aux_classify((const uint8_t*)c->scratch, c->code, c->g, c->stream) != cudaSuccess) {
+        aux_classify(c->Q, (const uint8_t*)c->scratch, c->code, c->mask, c->g, c->stream) != cudaSuccess) {
         set_err("classification launch failed: %s", cudaGetErrorString(cudaGetLastError()));
         lbm_destroy(c);
         return nullptr;
@@ -269,6 +272,7 @@ int lbm_destroy(lbm_t* c)
     dev_free(c, c->pop[0]);
     dev_free(c, c->pop[1]);
     dev_free(c, c->code);
+    dev_free(c, c->mask);
     dev_free(c, c->scratch);
     dev_free(c, c->partial);
     delete c;
@@ -285,7 +289,7 @@ int lbm_set_flags(lbm_t* c, const uint8_t* flags, const double u_wall[3])
     }
     for (int a = 0; a < 3; ++a) c->u_wall[a] = u_wall ? u_wall[a] : 0.0;
     CK(cudaMemcpyAsync(c->scratch, flags, (size_t)c->g.n, cudaMemcpyHostToDevice, c->stream));
-    CK(aux_classify((const uint8_t*)c->scratch, c->code, c->g, c->stream));
+    CK(aux_classify(c->Q, (const uint8_t*)c->scratch, c->code, c->mask, c->g, c->stream));
     c->launches++;
     CK(cudaStreamSynchronize(c->stream));
     c->n_fluid = nfluid;
@@ -420,13 +424,13 @@ int lbm_kinetic_energy(lbm_t* c, double* e)
     return LBM_OK;
 }
 
-int lbm_get_populations(lbm_t* c, void* f)
+// canonical planes f_k of the whole box (cells_dev == nullptr, m = N) or of m listed cells
+static int export_planes(lbm_t* c, void* f, const int* cells_dev, int m)
 {
-    if (!c || !f) { set_err("null argument"); return LBM_E_ARG; }
-    if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
-    const size_t nb = (size_t)c->g.n * c->elem;
+    const size_t nb = (size_t)m * c->elem;
+    const size_t plane = (size_t)c->g.n * c->elem;
     const int mode = load_mode(c);
-    // two scratch planes alternate so that the copy of plane k overlaps nothing it still needs
+    // scratch planes alternate so that the copy of plane k overlaps nothing it still needs
     for (int k = 0; k < c->Q; ++k) {
         const int kb = c->opp[k];
         PlaneArgs p;
@@ -439,16 +443,43 @@ int lbm_get_populations(lbm_t* c, void* f)
             p.slot_wall = mode == LD_PULL ? kb : k;
             p.sx = c->c[k][0]; p.sy = c->c[k][1]; p.sz = c->c[k][2];
         }
-        char* out = (char*)c->scratch + (size_t)(k & 3) * nb;
+        char* out = (char*)c->scratch + (size_t)(k & 3) * plane;
         if (c->dtype == LBM_F64)
-            CK(aux_extract_plane<double>(c->Q, c->soa, (const double*)c->pop[0], c->code, c->g, p, (double*)out, c->stream));
+            CK(aux_extract_plane<double>(c->Q, c->soa, (const double*)c->pop[0], c->code, c->g, p, (double*)out, cells_dev, m, c->stream));
         else
-            CK(aux_extract_plane<float>(c->Q, c->soa, (const float*)c->pop[0], c->code, c->g, p, (float*)out, c->stream));
+            CK(aux_extract_plane<float>(c->Q, c->soa, (const float*)c->pop[0], c->code, c->g, p, (float*)out, cells_dev, m, c->stream));
         c->launches++;
         CK(cudaMemcpyAsync((char*)f + (size_t)k * nb, out, nb, cudaMemcpyDeviceToHost, c->stream));
     }
     CK(cudaStreamSynchronize(c->stream));
     return LBM_OK;
+}
+
+int lbm_get_populations(lbm_t* c, void* f)
+{
+    if (!c || !f) { set_err("null argument"); return LBM_E_ARG; }
+    if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
+    return export_planes(c, f, nullptr, c->g.n);
+}
+
+int lbm_get_populations_at(lbm_t* c, const int32_t* cells, int m, void* f)
+{
+    if (!c || !f || (!cells && m > 0)) { set_err("null argument"); return LBM_E_ARG; }
+    if (m < 0 || m > c->g.n) { set_err("m must be in [0, N]"); return LBM_E_ARG; }
+    if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
+    if (m == 0) return LBM_OK;
+    for (int t = 0; t < m; ++t)
+        if (cells[t] < 0 || cells[t] >= c->g.n) { set_err("cell index %d out of range at position %d", cells[t], t); return LBM_E_ARG; }
+    int* cells_dev = (int*)dev_alloc(c, sizeof(int) * (size_t)m);
+    if (!cells_dev) { set_err("device allocation failed"); return LBM_E_ALLOC; }
+    c->dev_bytes -= (long long)(sizeof(int) * (size_t)m);  // transient
+    int rc = LBM_OK;
+    if (cudaMemcpyAsync(cells_dev, cells, sizeof(int) * (size_t)m, cudaMemcpyHostToDevice, c->stream) != cudaSuccess)
+        rc = cuda_fail("cell list upload", cudaGetLastError());
+    if (rc == LBM_OK) rc = export_planes(c, f, cells_dev, m);
+    cudaStreamSynchronize(c->stream);
+    dev_free(c, cells_dev);
+    return rc;
 }
 
 int lbm_set_populations(lbm_t* c, const void* f)
@@ -478,6 +509,14 @@ int lbm_sync(lbm_t* c)
 {
     if (!c) { set_err("null context"); return LBM_E_ARG; }
     CK(cudaStreamSynchronize(c->stream));
+    return LBM_OK;
+}
+
+int lbm_set_block(lbm_t* c, int threads)
+{
+    if (!c) { set_err("null context"); return LBM_E_ARG; }
+    if (threads < 32 || threads > 256 || (threads & 31)) { set_err("threads per block must be a multiple of 32 in [32, 256]"); return LBM_E_ARG; }
+    c->block = threads;
     return LBM_OK;
 }
 
