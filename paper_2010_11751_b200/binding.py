@@ -11,7 +11,8 @@ import os
 import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "liblbm_b200.so")
+# LBM_B200_LIB selects another build of the same library (tuning variants of build.py --out)
+LIB_PATH = os.environ.get("LBM_B200_LIB") or os.path.join(HERE, "liblbm_b200.so")
 
 LATTICES = {"D3Q19": 19, "D3Q27": 27, 19: 19, 27: 27}
 MODELS = {"BGK_W2": 0, "BGK_NW4": 1, "TRT": 2, "RM": 3, "HM": 4, "CM": 5, "CHM": 6, "K": 7, "RR": 8, "REG": 9}

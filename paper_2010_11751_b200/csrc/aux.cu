@@ -64,8 +64,8 @@ __global__ void __launch_bounds__(256) stream_only_kernel(const StepArgs<T> a)
     const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
     if (!cs.active) return;
     T f[Q];
-    load_cell<T, Q, SOA, LD_PULL>(a.src, a.g, a.wterm, i, cs.masked, cs.mask, f);
-    store_cell<T, Q, SOA, ST_LOCAL>(a.dst, a.g, a.wterm, i, cs.masked, cs.mask, f);
+    load_cell<T, Q, SOA, LD_PULL>(a, i, cs.masked, cs.mask, f);
+    store_cell<T, Q, SOA, ST_LOCAL>(a, i, cs.masked, cs.mask, f);
 }
 
 static inline int blocks_for(int n, int block) { return (n + block - 1) / block; }

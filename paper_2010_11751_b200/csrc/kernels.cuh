@@ -47,6 +47,15 @@ struct StepArgs {
     Geo g;
     Rates<T> rt;
     T wterm[27];  // w_k
+    // offsets filled on the host per launch (make_args) so that the kernels add one uniform
+    // 64-bit constant per direction instead of multiplying strides per thread:
+    //   plane[k]  slot k of cell 0, in elements          (SoA: k*stride, AoS: k)
+    //   ldo[k]    where the pure load of f_k starts, in BYTES: LD_LOCAL plane[k]; LD_PULL
+    //             plane[k] - off_k*IS; LD_AAPULL plane[kbar] - off_k*IS   (times sizeof(T))
+    //   sto[k]    where the pure store of f_k goes, in BYTES: ST_LOCAL plane[k]; ST_SWAPPED
+    //             plane[kbar]; ST_PUSH plane[k] + off_k*IS                (times sizeof(T))
+    // with IS = 1 (SoA) or Q (AoS) elements per cell step and off_k the cell-index offset of c_k.
+    long long plane[27], ldo[27], sto[27];
 };
 
 template <bool SOA, int Q>
@@ -107,32 +116,28 @@ struct Edge {
 // ------------------------------------------------------------------ load / store of one cell
 // `masked` must be warp-uniform; mask is this cell's link mask (0 for a bulk cell)
 template <class T, int Q, bool SOA, int LOAD>
-__device__ __forceinline__ void load_cell(const T* __restrict__ src, const Geo& g, const T (&wterm)[27], int i,
-                                          bool masked, unsigned long long mask, T (&f)[Q])
+__device__ __forceinline__ void load_cell(const StepArgs<T>& a, int i, bool masked, unsigned long long mask, T (&f)[Q])
 {
     using L = Lat<Q>;
-    if (LOAD == LD_LOCAL) {
-        static_for<Q>([&](auto kc) { f[kc] = src[slot<SOA, Q>(g, kc, i)]; });
-    } else if (!masked) {
-        static_for<Q>([&](auto kc) {
-            constexpr int k = kc;
-            constexpr int s = LOAD == LD_PULL ? k : L::opp(k);
-            f[k] = src[slot<SOA, Q>(g, s, (long long)i - offset<Q, k>(g))];
-        });
+    constexpr int IS = SOA ? 1 : Q;
+    const T* __restrict__ src = a.src;
+    if (LOAD == LD_LOCAL || !masked) {
+        const char* __restrict__ p = reinterpret_cast<const char*>(src + (long long)i * IS);
+        static_for<Q>([&](auto kc) { f[kc] = *reinterpret_cast<const T*>(p + a.ldo[kc]); });
     } else {
-        const Edge e(mask, g);
+        const Edge e(mask, a.g);
         static_for<Q>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
             if constexpr (k == L::REST) {
-                f[k] = src[slot<SOA, Q>(g, k, i)];
+                f[k] = src[a.plane[k] + (long long)i * IS];
             } else {
                 // the upstream neighbour x - c_k = x + c_kbar
                 constexpr int s_fluid = LOAD == LD_PULL ? k : kb, s_wall = LOAD == LD_PULL ? kb : k;
                 const bool sol = e.template solid<Q, kb>();
-                const long long a_fluid = slot<SOA, Q>(g, s_fluid, (long long)i + e.template off<Q, k, -1>());
-                const long long a_wall = slot<SOA, Q>(g, s_wall, i);
+                const long long a_fluid = a.plane[s_fluid] + (long long)(i + e.template off<Q, k, -1>()) * IS;
+                const long long a_wall = a.plane[s_wall] + (long long)i * IS;
                 T v = src[sol ? a_wall : a_fluid];
-                if (e.template moving<Q, kb>()) v += wterm[kb];
+                if (e.template moving<Q, kb>()) v += a.wterm[kb];
                 f[k] = v;
             }
         });
@@ -140,31 +145,26 @@ __device__ __forceinline__ void load_cell(const T* __restrict__ src, const Geo& 
 }
 
 template <class T, int Q, bool SOA, int STORE>
-__device__ __forceinline__ void store_cell(T* __restrict__ dst, const Geo& g, const T (&wterm)[27], int i, bool masked,
-                                           unsigned long long mask, const T (&f)[Q])
+__device__ __forceinline__ void store_cell(const StepArgs<T>& a, int i, bool masked, unsigned long long mask, const T (&f)[Q])
 {
     using L = Lat<Q>;
-    if (STORE == ST_LOCAL) {
-        static_for<Q>([&](auto kc) { dst[slot<SOA, Q>(g, kc, i)] = f[kc]; });
-    } else if (STORE == ST_SWAPPED) {
-        static_for<Q>([&](auto kc) { dst[slot<SOA, Q>(g, L::opp(kc), i)] = f[kc]; });
-    } else if (!masked) {
-        static_for<Q>([&](auto kc) {
-            constexpr int k = kc;
-            dst[slot<SOA, Q>(g, k, (long long)i + offset<Q, k>(g))] = f[k];
-        });
+    constexpr int IS = SOA ? 1 : Q;
+    T* __restrict__ dst = a.dst;
+    if (STORE != ST_PUSH || !masked) {
+        char* __restrict__ p = reinterpret_cast<char*>(dst + (long long)i * IS);
+        static_for<Q>([&](auto kc) { *reinterpret_cast<T*>(p + a.sto[kc]) = f[kc]; });
     } else {
-        const Edge e(mask, g);
+        const Edge e(mask, a.g);
         static_for<Q>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
             if constexpr (k == L::REST) {
-                dst[slot<SOA, Q>(g, k, i)] = f[k];
+                dst[a.plane[k] + (long long)i * IS] = f[k];
             } else {
                 const bool sol = e.template solid<Q, k>();
-                const long long a_fluid = slot<SOA, Q>(g, k, (long long)i + e.template off<Q, k, +1>());
-                const long long a_wall = slot<SOA, Q>(g, kb, i);
+                const long long a_fluid = a.plane[k] + (long long)(i + e.template off<Q, k, +1>()) * IS;
+                const long long a_wall = a.plane[kb] + (long long)i * IS;
                 T v = f[k];
-                if (e.template moving<Q, k>()) v += wterm[k];
+                if (e.template moving<Q, k>()) v += a.wterm[k];
                 dst[sol ? a_wall : a_fluid] = v;
             }
         });
@@ -190,17 +190,30 @@ __device__ __forceinline__ CellState cell_state(const uint8_t* __restrict__ code
 }
 
 // ------------------------------------------------------------------ the fused step
+// minimum resident blocks of 256 threads per SM (register cap 65536 / (256 * n)): tuned on B200
+#ifndef LBM_MINB_D19
+#define LBM_MINB_D19 3
+#endif
+#ifndef LBM_MINB_D27
+#define LBM_MINB_D27 2
+#endif
+#ifndef LBM_MINB_F
+#define LBM_MINB_F 6
+#endif
+template <class T, int Q>
+constexpr int min_blocks() { return sizeof(T) == 4 ? LBM_MINB_F : Q == 19 ? LBM_MINB_D19 : LBM_MINB_D27; }
+
 template <class T, int Q, int MODEL, bool SOA, int LOAD, int STORE>
-__global__ void __launch_bounds__(256) step_kernel(const StepArgs<T> a)
+__global__ void __launch_bounds__(256, min_blocks<T, Q>()) step_kernel(const StepArgs<T> a)
 {
     constexpr bool SHIFT = sizeof(T) == 4;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
     if (!cs.active) return;  // solid cells hold no populations
     T f[Q];
-    load_cell<T, Q, SOA, LOAD>(a.src, a.g, a.wterm, i, cs.masked, cs.mask, f);
+    load_cell<T, Q, SOA, LOAD>(a, i, cs.masked, cs.mask, f);
     collide<Q, MODEL, SHIFT>(f, a.rt);
-    store_cell<T, Q, SOA, STORE>(a.dst, a.g, a.wterm, i, cs.masked, cs.mask, f);
+    store_cell<T, Q, SOA, STORE>(a, i, cs.masked, cs.mask, f);
 }
 
 // ------------------------------------------------------------------ swap scheme, pass 2
@@ -295,7 +308,7 @@ __global__ void macroscopic_kernel(const T* __restrict__ pop, const uint8_t* __r
     T r = T(0), uu[3] = {T(0), T(0), T(0)};
     if (cs.active) {
         T f[Q], dr;
-        load_cell<T, Q, SOA, LOAD>(pop, g, a.wterm, i, cs.masked, cs.mask, f);
+        load_cell<T, Q, SOA, LOAD>(a, i, cs.masked, cs.mask, f);
         moments_rho_u<Q, SHIFT>(f, r, dr, uu);
     }
     rho[i] = r;
@@ -317,7 +330,7 @@ __global__ void __launch_bounds__(256) energy_kernel(const T* __restrict__ pop, 
         const CellState cs = cell_state(code, a.mask, i, g.n);
         if (!cs.active) continue;
         T f[Q], r, dr, uu[3];
-        load_cell<T, Q, SOA, LOAD>(pop, g, a.wterm, (int)i, cs.masked, cs.mask, f);
+        load_cell<T, Q, SOA, LOAD>(a, (int)i, cs.masked, cs.mask, f);
         moments_rho_u<Q, SHIFT>(f, r, dr, uu);
         e += 0.5 * (double)r * ((double)uu[0] * uu[0] + (double)uu[1] * uu[1] + (double)uu[2] * uu[2]);
     }

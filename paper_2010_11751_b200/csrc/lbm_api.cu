@@ -93,10 +93,34 @@ int cuda_fail(const char* what, cudaError_t e)
         if (e_ != cudaSuccess) return cuda_fail(#call, e_); \
     } while (0)
 
+// load / store modes of a step-kernel kind (kernels.cuh)
+void kind_modes(int kind, int* load, int* store)
+{
+    switch (kind) {
+    case SK_PUSH: *load = LD_LOCAL; *store = ST_PUSH; break;
+    case SK_PULL: *load = LD_PULL; *store = ST_LOCAL; break;
+    case SK_COLLIDE: *load = LD_LOCAL; *store = ST_LOCAL; break;
+    case SK_EVEN: *load = LD_LOCAL; *store = ST_SWAPPED; break;
+    default: *load = LD_AAPULL; *store = ST_PUSH; break;
+    }
+}
+
 template <class T>
-StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst)
+StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = LD_LOCAL, int store = ST_LOCAL)
 {
     StepArgs<T> a;
+    const long long is = c->soa ? 1 : c->Q;  // elements per cell step
+    for (int k = 0; k < 27; ++k) {
+        a.plane[k] = a.ldo[k] = a.sto[k] = 0;
+        if (k >= c->Q) continue;
+        const int kb = c->opp[k];
+        const long long off = ((long long)c->c[k][0] * c->ny + c->c[k][1]) * c->nz + c->c[k][2];
+        const long long pk = c->soa ? (long long)k * c->g.stride : k;
+        const long long pkb = c->soa ? (long long)kb * c->g.stride : kb;
+        a.plane[k] = pk;
+        a.ldo[k] = (long long)sizeof(T) * (load == LD_LOCAL ? pk : load == LD_PULL ? pk - off * is : pkb - off * is);
+        a.sto[k] = (long long)sizeof(T) * (store == ST_LOCAL ? pk : store == ST_SWAPPED ? pkb : pk + off * is);
+    }
     a.src = (const T*)src;
     a.dst = (T*)dst;
     a.code = c->code;
@@ -146,7 +170,9 @@ cudaError_t step_model(const lbm_ctx* c, int kind, const StepArgs<T>& a)
 template <class T>
 cudaError_t step_kind(lbm_ctx* c, int kind, const void* src, void* dst)
 {
-    StepArgs<T> a = make_args<T>(c, src, dst);
+    int load, store;
+    kind_modes(kind, &load, &store);
+    StepArgs<T> a = make_args<T>(c, src, dst, load, store);
     c->launches++;
     return c->Q == 19 ? step_model<T, 19>(c, kind, a) : step_model<T, 27>(c, kind, a);
 }
@@ -168,8 +194,8 @@ int normalise(lbm_ctx* c)
 {
     if (c->sto != STO_POST) return LBM_OK;
     cudaError_t e;
-    if (c->dtype == LBM_F64) e = aux_stream_only<double>(c->Q, c->soa, make_args<double>(c, c->pop[0], c->pop[1]), c->stream);
-    else e = aux_stream_only<float>(c->Q, c->soa, make_args<float>(c, c->pop[0], c->pop[1]), c->stream);
+    if (c->dtype == LBM_F64) e = aux_stream_only<double>(c->Q, c->soa, make_args<double>(c, c->pop[0], c->pop[1], LD_PULL, ST_LOCAL), c->stream);
+    else e = aux_stream_only<float>(c->Q, c->soa, make_args<float>(c, c->pop[0], c->pop[1], LD_PULL, ST_LOCAL), c->stream);
     c->launches++;
     if (e != cudaSuccess) return cuda_fail("stream_only", e);
     void* t = c->pop[0]; c->pop[0] = c->pop[1]; c->pop[1] = t;
@@ -387,10 +413,10 @@ int lbm_macroscopic_device(lbm_t* c, void* rho, void* u)
     if (!c || !rho || !u) { set_err("null argument"); return LBM_E_ARG; }
     if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
     if (c->dtype == LBM_F64)
-        CK(aux_macroscopic<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr), (double*)rho,
+        CK(aux_macroscopic<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr, load_mode(c)), (double*)rho,
                                    (double*)u, c->stream));
     else
-        CK(aux_macroscopic<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr), (float*)rho,
+        CK(aux_macroscopic<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr, load_mode(c)), (float*)rho,
                                   (float*)u, c->stream));
     c->launches++;
     return LBM_OK;
@@ -413,10 +439,10 @@ int lbm_kinetic_energy(lbm_t* c, double* e)
     if (!c || !e) { set_err("null argument"); return LBM_E_ARG; }
     if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
     if (c->dtype == LBM_F64)
-        CK(aux_energy<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr), c->partial,
+        CK(aux_energy<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr, load_mode(c)), c->partial,
                               c->n_partial, c->e_dev, c->stream));
     else
-        CK(aux_energy<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr), c->partial,
+        CK(aux_energy<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr, load_mode(c)), c->partial,
                              c->n_partial, c->e_dev, c->stream));
     c->launches += 2;
     CK(cudaMemcpyAsync(e, c->e_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
