@@ -119,6 +119,15 @@ int lbm_set_variant(lbm_t* ctx, int variant);
  * default 128).  Results do not depend on it. */
 int lbm_set_block(lbm_t* ctx, int threads);
 
+/* CUDA-graph replay of lbm_step.  A step of a lattice below ~96^3 cells lasts a few microseconds
+ * and is bound by launch latency (the paper's "one synchronisation per step");
+ * lbm_step(n) then captures 16 steps once and replays the graph.  LBM_GRAPH_AUTO (default): only
+ * for such small lattices; LBM_GRAPH_OFF: never; LBM_GRAPH_ON: for any size.  Results are
+ * identical (same kernels, same order).  lbm_graph_replays = graph launches so far. */
+enum { LBM_GRAPH_AUTO = 0, LBM_GRAPH_OFF = 1, LBM_GRAPH_ON = 2 };
+int lbm_set_graph(lbm_t* ctx, int mode);
+long long lbm_graph_replays(const lbm_t* ctx);
+
 const char* lbm_last_error(void);
 const char* lbm_version(void);
 

@@ -27,8 +27,9 @@ SYMBOLS = [
     "lbm_set_hooks", "lbm_create", "lbm_destroy", "lbm_set_flags", "lbm_set_relaxation", "lbm_set_trt_magic",
     "lbm_init_equilibrium", "lbm_init_equilibrium_device", "lbm_step", "lbm_macroscopic", "lbm_macroscopic_device", "lbm_kinetic_energy", "lbm_get_populations", "lbm_get_populations_at",
     "lbm_set_populations", "lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches",
-    "lbm_sync", "lbm_set_variant", "lbm_set_block", "lbm_last_error", "lbm_version",
+    "lbm_sync", "lbm_set_variant", "lbm_set_block", "lbm_set_graph", "lbm_graph_replays", "lbm_last_error", "lbm_version",
 ]
+GRAPH_MODES = {"auto": 0, "off": 1, "on": 2}
 
 
 class LbmError(RuntimeError):
@@ -68,7 +69,8 @@ def load_library(path=LIB_PATH):
     L.lbm_get_populations.argtypes = [vp, vp]
     L.lbm_get_populations_at.argtypes = [vp, vp, i, vp]
     L.lbm_set_populations.argtypes = [vp, vp]
-    for name in ("lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches"):
+    L.lbm_set_graph.argtypes = [vp, i]
+    for name in ("lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches", "lbm_graph_replays"):
         getattr(L, name).restype = C.c_longlong
         getattr(L, name).argtypes = [vp]
     L.lbm_sync.argtypes = [vp]
@@ -229,3 +231,11 @@ class Lbm:
     @property
     def kernel_launches(self):
         return self._L.lbm_kernel_launches(self._h)
+
+    @property
+    def graph_replays(self):
+        return self._L.lbm_graph_replays(self._h)
+
+    def set_graph(self, mode):
+        """CUDA-graph replay of step(): "auto" (small lattices only), "off", "on"."""
+        self._ck(self._L.lbm_set_graph(self._h, GRAPH_MODES[mode]))

@@ -38,21 +38,23 @@ __global__ void classify_kernel(const uint8_t* __restrict__ flags, uint8_t* __re
     mask[i] = m;
 }
 
-// energy stage 2: one block sums the per-block partials in a fixed order
-__global__ void __launch_bounds__(1024) energy_final_kernel(const double* __restrict__ partial, int n, double* __restrict__ out)
+// energy stages 2 and 3: block b sums the contiguous segment [b*seg, min(n, (b+1)*seg)) of `in` in a
+// fixed order into out[b]; launched once with many blocks and once with a single block
+__global__ void __launch_bounds__(256) energy_sum_kernel(const double* __restrict__ in, int n, int seg, double* __restrict__ out)
 {
-    __shared__ double ws[32];
+    __shared__ double ws[8];
+    const int lo = blockIdx.x * seg, hi = min(n, lo + seg);
     double e = 0.0;
-    for (int i = threadIdx.x; i < n; i += 1024) e += partial[i];
+    for (int i = lo + threadIdx.x; i < hi; i += 256) e += in[i];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) e += __shfl_down_sync(0xffffffffu, e, o);
     if ((threadIdx.x & 31) == 0) ws[threadIdx.x >> 5] = e;
     __syncthreads();
     if (threadIdx.x < 32) {
-        e = ws[threadIdx.x];
+        e = threadIdx.x < 8 ? ws[threadIdx.x] : 0.0;
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) e += __shfl_down_sync(0xffffffffu, e, o);
-        if (threadIdx.x == 0) *out = e;
+        for (int o = 4; o > 0; o >>= 1) e += __shfl_down_sync(0xffffffffu, e, o);
+        if (threadIdx.x == 0) out[blockIdx.x] = e;
     }
 }
 
@@ -117,6 +119,7 @@ cudaError_t aux_macroscopic(int Q, bool soa, int load, const StepArgs<T>& a, T* 
     return cudaGetLastError();
 }
 
+// partial: [nblocks + ENERGY_STAGE2] doubles, nblocks = ceil(n / 256); out: one double
 template <class T>
 cudaError_t aux_energy(int Q, bool soa, int load, const StepArgs<T>& a, double* partial, int nblocks, double* out,
                        cudaStream_t s)
@@ -132,7 +135,10 @@ cudaError_t aux_energy(int Q, bool soa, int load, const StepArgs<T>& a, double* 
 #undef CALL
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    energy_final_kernel<<<1, 1024, 0, s>>>(partial, nblocks, out);
+    const int seg = (nblocks + ENERGY_STAGE2 - 1) / ENERGY_STAGE2;
+    const int n2 = (nblocks + seg - 1) / seg;
+    energy_sum_kernel<<<n2, 256, 0, s>>>(partial, nblocks, seg, partial + nblocks);
+    energy_sum_kernel<<<1, 256, 0, s>>>(partial + nblocks, n2, n2, out);
     return cudaGetLastError();
 }
 

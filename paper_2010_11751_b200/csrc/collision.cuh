@@ -299,20 +299,22 @@ __device__ __forceinline__ void collide(T (&f)[Q], const Rates<T>& rt)
         const T e0 = SHIFT ? t0 * (drho - rho * usq15) : t0 * rho * (T(1) - usq15);
         f[L::REST] = omc * f[L::REST] + om * e0;
     } else if constexpr (MODEL == M_TRT) {
-        // symmetric part relaxed with omega+, antisymmetric with omega- (R15)
+        // symmetric part relaxed with omega+, antisymmetric with omega- (R15):
+        //   f_k' = f_k - w+ (fs - Es) - w- (fa - Ea),  fs = (f_k + f_kbar)/2, fa = (f_k - f_kbar)/2
+        //        = a f_k + b f_kbar + (w+ Es + w- Ea),  a = 1 - (w+ + w-)/2, b = (w- - w+)/2
         const T usq15 = T(1.5) * (u[0] * u[0] + u[1] * u[1] + u[2] * u[2]);
         const T wp = rt.omega, wm = rt.omega_minus;
+        const T ca = T(1) - T(0.5) * (wp + wm), cb = T(0.5) * (wm - wp);
         static_for<L::NH>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
             const T tk = T(L::w(k));
             const T cu = c_dot<Q, k>(u);
             const T quad = T(4.5) * cu * cu - usq15;
-            const T esym = SHIFT ? tk * (drho + rho * quad) : tk * rho * (T(1) + quad);
-            const T easym = T(3) * tk * rho * cu;
-            const T fs = T(0.5) * (f[k] + f[kb]), fa = T(0.5) * (f[k] - f[kb]);
-            const T ds = wp * (fs - esym), da = wm * (fa - easym);
-            f[k] = f[k] - ds - da;
-            f[kb] = f[kb] - ds + da;
+            const T esym = wp * (SHIFT ? tk * (drho + rho * quad) : tk * rho * (T(1) + quad));
+            const T easym = wm * (T(3) * tk * rho * cu);
+            const T fk = f[k], fb = f[kb];
+            f[k] = ca * fk + cb * fb + (esym + easym);
+            f[kb] = ca * fb + cb * fk + (esym - easym);
         });
         const T t0 = T(L::w(L::REST));
         const T e0 = SHIFT ? t0 * (drho - rho * usq15) : t0 * rho * (T(1) - usq15);

@@ -35,6 +35,7 @@ cudaError_t aux_init_equilibrium(int Q, bool ext, bool soa, T* pop, const uint8_
                                  const T* u, cudaStream_t s);
 template <class T>
 cudaError_t aux_macroscopic(int Q, bool soa, int load, const StepArgs<T>& a, T* rho, T* u, cudaStream_t s);
+enum { ENERGY_STAGE2 = 512 };  // blocks of the second reduction stage
 template <class T>
 cudaError_t aux_energy(int Q, bool soa, int load, const StepArgs<T>& a, double* partial, int nblocks, double* out,
                        cudaStream_t s);

@@ -200,8 +200,11 @@ __device__ __forceinline__ CellState cell_state(const uint8_t* __restrict__ code
 #ifndef LBM_MINB_F
 #define LBM_MINB_F 6
 #endif
+#ifndef LBM_MINB_F27
+#define LBM_MINB_F27 4
+#endif
 template <class T, int Q>
-constexpr int min_blocks() { return sizeof(T) == 4 ? LBM_MINB_F : Q == 19 ? LBM_MINB_D19 : LBM_MINB_D27; }
+constexpr int min_blocks() { return sizeof(T) == 4 ? (Q == 19 ? LBM_MINB_F : LBM_MINB_F27) : Q == 19 ? LBM_MINB_D19 : LBM_MINB_D27; }
 
 template <class T, int Q, int MODEL, bool SOA, int LOAD, int STORE>
 __global__ void __launch_bounds__(256, min_blocks<T, Q>()) step_kernel(const StepArgs<T> a)
@@ -222,8 +225,14 @@ __global__ void __launch_bounds__(256, min_blocks<T, Q>()) step_kernel(const Ste
 // in the slot Eq 3 sends it to); and when the neighbour at x - c_k is a wall, add w_kbar to pop_k(x).
 // Every slot is touched by exactly one thread (Table 1), so all loads
 // are issued before the first store.
+#ifndef LBM_MINB_SWAP
+#define LBM_MINB_SWAP 3
+#endif
+#ifndef LBM_MINB_SWAP_D27
+#define LBM_MINB_SWAP_D27 2
+#endif
 template <class T, int Q, bool SOA>
-__global__ void __launch_bounds__(256) swap_stream_kernel(const StepArgs<T> a)
+__global__ void __launch_bounds__(256, (Q == 27 && sizeof(T) == 8) ? LBM_MINB_SWAP_D27 : LBM_MINB_SWAP) swap_stream_kernel(const StepArgs<T> a)
 {
     using L = Lat<Q>;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -317,22 +326,21 @@ __global__ void macroscopic_kernel(const T* __restrict__ pop, const uint8_t* __r
     u[2LL * g.n + i] = uu[2];
 }
 
-// kinetic energy, stage 1: one double per block (fixed tree: warp shuffle, then warp 0)
+// kinetic energy, stage 1: one cell per thread, one double per block of 256 cells (fixed tree: warp
+// shuffle, then warp 0), so that as many loads are in flight as in the step kernels
 template <class T, int Q, bool SOA, int LOAD>
-__global__ void __launch_bounds__(256) energy_kernel(const T* __restrict__ pop, const uint8_t* __restrict__ code, Geo g,
-                                                     StepArgs<T> a, double* __restrict__ partial)
+__global__ void __launch_bounds__(256, min_blocks<T, Q>()) energy_kernel(const T* __restrict__ pop, const uint8_t* __restrict__ code, Geo g,
+                                                                         StepArgs<T> a, double* __restrict__ partial)
 {
     constexpr bool SHIFT = sizeof(T) == 4;
     double e = 0.0;
-    // the trip count is the same for every lane of a warp (cell_state votes across the warp)
-    const long long n32 = ((long long)g.n + 31) & ~31LL;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n32; i += (long long)gridDim.x * blockDim.x) {
-        const CellState cs = cell_state(code, a.mask, i, g.n);
-        if (!cs.active) continue;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const CellState cs = cell_state(code, a.mask, i, g.n);
+    if (cs.active) {
         T f[Q], r, dr, uu[3];
-        load_cell<T, Q, SOA, LOAD>(a, (int)i, cs.masked, cs.mask, f);
+        load_cell<T, Q, SOA, LOAD>(a, i, cs.masked, cs.mask, f);
         moments_rho_u<Q, SHIFT>(f, r, dr, uu);
-        e += 0.5 * (double)r * ((double)uu[0] * uu[0] + (double)uu[1] * uu[1] + (double)uu[2] * uu[2]);
+        e = 0.5 * (double)r * ((double)uu[0] * uu[0] + (double)uu[1] * uu[1] + (double)uu[2] * uu[2]);
     }
     __shared__ double ws[8];
 #pragma unroll

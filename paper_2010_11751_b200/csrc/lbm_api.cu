@@ -63,6 +63,12 @@ struct lbm_ctx {
     cudaStream_t stream;
     int c[27][3], opp[27];
     double w[27];
+    // CUDA-graph replay of lbm_step for launch-bound lattices (see step_graphed)
+    int graph_mode;             // LBM_GRAPH_AUTO / OFF / ON
+    cudaGraphExec_t graph_exec; // GRAPH_STEPS steps starting from graph_sto with pop[0] == graph_pop0
+    Storage graph_sto;
+    void* graph_pop0;
+    long long graph_replays;
 };
 
 namespace {
@@ -203,6 +209,103 @@ int normalise(lbm_ctx* c)
     return LBM_OK;
 }
 
+// one collide-and-stream cycle by the context's scheme (Table 1)
+int one_step(lbm_ctx* c)
+{
+    if (c->fam == FAM_2POP) {
+        if (use_pull(c)) {
+            if (c->sto == STO_CANON) {  // (S C)^n = S (C S)^(n-1) C: start with a collide-only pass
+                CK(step_kind(c, SK_COLLIDE, c->pop[0], c->pop[0]));
+                c->sto = STO_POST;
+            } else {
+                CK(step_kind(c, SK_PULL, c->pop[0], c->pop[1]));
+                void* t = c->pop[0]; c->pop[0] = c->pop[1]; c->pop[1] = t;
+            }
+        } else {
+            if (int rc = normalise(c)) return rc;
+            CK(step_kind(c, SK_PUSH, c->pop[0], c->pop[1]));
+            void* t = c->pop[0]; c->pop[0] = c->pop[1]; c->pop[1] = t;
+        }
+    } else if (c->fam == FAM_AA) {
+        if (c->sto == STO_CANON) {
+            CK(step_kind(c, SK_EVEN, c->pop[0], c->pop[0]));
+            c->sto = STO_AA_ODD;
+        } else {
+            CK(step_kind(c, SK_ODD, c->pop[0], c->pop[0]));
+            c->sto = STO_CANON;
+        }
+    } else {
+        CK(step_kind(c, SK_EVEN, c->pop[0], c->pop[0]));  // pass 1: collide into opposite slots
+        if (c->dtype == LBM_F64) CK(aux_swap_stream<double>(c->Q, c->soa, make_args<double>(c, c->pop[0], c->pop[0]), c->stream));
+        else CK(aux_swap_stream<float>(c->Q, c->soa, make_args<float>(c, c->pop[0], c->pop[0]), c->stream));
+        c->launches++;
+    }
+    c->steps++;
+    return LBM_OK;
+}
+
+// ---- CUDA-graph replay.  Below ~64^3 cells a step kernel runs for a few microseconds and the
+// time step is bound by launch latency (one launch per step, two for swap; "one
+// synchronisation per step").  GRAPH_STEPS steps are captured once into a graph (kernel arguments
+// baked in) and replayed; every scheme returns to the same storage state and the same pop[0]
+// after an even number of steps, so one graph serves the whole run.  Any call that changes what
+// the kernels would be given (rates, flags, variant, block, populations' home) drops the graph.
+enum { GRAPH_STEPS = 16, GRAPH_AUTO_MAX_CELLS = 96 * 96 * 96 };
+
+void drop_graph(lbm_ctx* c)
+{
+    if (c->graph_exec) cudaGraphExecDestroy(c->graph_exec);
+    c->graph_exec = nullptr;
+}
+
+bool graph_wanted(const lbm_ctx* c, int n)
+{
+    if (n < GRAPH_STEPS || c->graph_mode == LBM_GRAPH_OFF) return false;
+    return c->graph_mode == LBM_GRAPH_ON || c->g.n <= GRAPH_AUTO_MAX_CELLS;
+}
+
+// run GRAPH_STEPS steps through the cached graph (capturing it first if needed)
+int step_graphed(lbm_ctx* c)
+{
+    if (c->fam == FAM_2POP && use_pull(c) && c->sto == STO_CANON) return LBM_E_STATE;  // first step differs from the rest
+    if (c->graph_exec && (c->graph_sto != c->sto || c->graph_pop0 != c->pop[0])) drop_graph(c);
+    if (!c->graph_exec) {
+        cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(c->stream, &st) != cudaSuccess || st != cudaStreamCaptureStatusNone) {
+            cudaGetLastError();
+            return LBM_E_STATE;  // the caller is capturing this stream itself
+        }
+        const Storage sto0 = c->sto;
+        void* const pop0 = c->pop[0];
+        const long long steps0 = c->steps, launches0 = c->launches;
+        if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return LBM_E_STATE; }
+        int rc = LBM_OK;
+        for (int s = 0; s < GRAPH_STEPS && rc == LBM_OK; ++s) rc = one_step(c);
+        cudaGraph_t graph = nullptr;
+        cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+        // nothing ran: undo the bookkeeping of the captured steps
+        c->steps = steps0; c->launches = launches0;
+        const bool periodic = c->sto == sto0 && c->pop[0] == pop0;
+        c->sto = sto0;
+        if (c->pop[0] != pop0) { void* t = c->pop[0]; c->pop[0] = c->pop[1]; c->pop[1] = t; }
+        if (rc != LBM_OK || e != cudaSuccess || !graph || !periodic) {
+            if (graph) cudaGraphDestroy(graph);
+            cudaGetLastError();
+            return LBM_E_STATE;
+        }
+        e = cudaGraphInstantiate(&c->graph_exec, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) { c->graph_exec = nullptr; cudaGetLastError(); return LBM_E_STATE; }
+        c->graph_sto = sto0;
+        c->graph_pop0 = pop0;
+    }
+    CK(cudaGraphLaunch(c->graph_exec, c->stream));
+    c->steps += GRAPH_STEPS;
+    c->launches += GRAPH_STEPS * (c->fam == FAM_SWAP ? 2 : 1);
+    c->graph_replays++;
+    return LBM_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -271,14 +374,14 @@ lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme
     if (ok) ok = cudaMemsetAsync(c->code, 0, (size_t)c->g.n, c->stream) == cudaSuccess;
     if (ok) { c->mask = (unsigned long long*)dev_alloc(c, sizeof(unsigned long long) * (size_t)c->g.n); ok = c->mask != nullptr; }
     if (ok) { c->scratch = dev_alloc(c, 4 * (size_t)c->g.n * c->elem); ok = c->scratch != nullptr; }
-    c->n_partial = 148 * 8;
-    if (ok) { c->partial = (double*)dev_alloc(c, sizeof(double) * (c->n_partial + 1)); ok = c->partial != nullptr; }
+    c->n_partial = (c->g.n + 255) / 256;  // one partial per block of 256 cells, then two fixed summing stages
+    if (ok) { c->partial = (double*)dev_alloc(c, sizeof(double) * (c->n_partial + ENERGY_STAGE2 + 1)); ok = c->partial != nullptr; }
     if (!ok) {
         set_err("device allocation failed (%lld bytes so far): %s", c->dev_bytes, cudaGetErrorString(cudaGetLastError()));
         lbm_destroy(c);
         return nullptr;
     }
-    c->e_dev = c->partial + c->n_partial;
+    c->e_dev = c->partial + c->n_partial + ENERGY_STAGE2;
     // cells on the faces of a fully periodic box still need the wrap: classify with all-fluid flags
     // (scratch is large enough to stand in for a zero flag array of N bytes)
     if (cudaMemsetAsync(c->scratch, 0, (size_t)c->g.n, c->stream) != cudaSuccess ||
@@ -295,6 +398,7 @@ int lbm_destroy(lbm_t* c)
 {
     if (!c) return LBM_OK;
     cudaStreamSynchronize(c->stream);
+    drop_graph(c);
     dev_free(c, c->pop[0]);
     dev_free(c, c->pop[1]);
     dev_free(c, c->code);
@@ -313,6 +417,7 @@ int lbm_set_flags(lbm_t* c, const uint8_t* flags, const double u_wall[3])
         if (flags[i] > LBM_MOVING) { set_err("flag %d at cell %d is not FLUID/WALL/MOVING", flags[i], i); return LBM_E_ARG; }
         nfluid += flags[i] == LBM_FLUID;
     }
+    drop_graph(c);
     for (int a = 0; a < 3; ++a) c->u_wall[a] = u_wall ? u_wall[a] : 0.0;
     CK(cudaMemcpyAsync(c->scratch, flags, (size_t)c->g.n, cudaMemcpyHostToDevice, c->stream));
     CK(aux_classify(c->Q, (const uint8_t*)c->scratch, c->code, c->mask, c->g, c->stream));
@@ -331,6 +436,7 @@ int lbm_set_relaxation(lbm_t* c, double omega_bulk, double omega3, double omega_
         return LBM_E_ARG;
     }
     c->omega_bulk = omega_bulk; c->omega3 = omega3; c->omega_hi = omega_hi;
+    drop_graph(c);
     return LBM_OK;
 }
 
@@ -338,6 +444,7 @@ int lbm_set_trt_magic(lbm_t* c, double lambda)
 {
     if (!c || !(lambda > 0.0)) { set_err("magic parameter must be positive"); return LBM_E_ARG; }
     c->trt_magic = lambda;
+    drop_graph(c);
     return LBM_OK;
 }
 
@@ -374,39 +481,33 @@ int lbm_step(lbm_t* c, int n)
     if (!c) { set_err("null context"); return LBM_E_ARG; }
     if (n < 0) { set_err("n must be >= 0"); return LBM_E_ARG; }
     if (c->sto == STO_NONE) { set_err("lbm_step before lbm_init_equilibrium / lbm_set_populations"); return LBM_E_STATE; }
-    for (int s = 0; s < n; ++s) {
-        if (c->fam == FAM_2POP) {
-            if (use_pull(c)) {
-                if (c->sto == STO_CANON) {  // (S C)^n = S (C S)^(n-1) C: start with a collide-only pass
-                    CK(step_kind(c, SK_COLLIDE, c->pop[0], c->pop[0]));
-                    c->sto = STO_POST;
-                } else {
-                    CK(step_kind(c, SK_PULL, c->pop[0], c->pop[1]));
-                    void* t = c->pop[0]; c->pop[0] = c->pop[1]; c->pop[1] = t;
-                }
-            } else {
-                if (int rc = normalise(c)) return rc;
-                CK(step_kind(c, SK_PUSH, c->pop[0], c->pop[1]));
-                void* t = c->pop[0]; c->pop[0] = c->pop[1]; c->pop[1] = t;  // PAPER.md:L126
-            }
-        } else if (c->fam == FAM_AA) {
-            if (c->sto == STO_CANON) {
-                CK(step_kind(c, SK_EVEN, c->pop[0], c->pop[0]));
-                c->sto = STO_AA_ODD;
-            } else {
-                CK(step_kind(c, SK_ODD, c->pop[0], c->pop[0]));
-                c->sto = STO_CANON;
-            }
-        } else {
-            CK(step_kind(c, SK_EVEN, c->pop[0], c->pop[0]));  // pass 1: collide into opposite slots
-            if (c->dtype == LBM_F64) CK(aux_swap_stream<double>(c->Q, c->soa, make_args<double>(c, c->pop[0], c->pop[0]), c->stream));
-            else CK(aux_swap_stream<float>(c->Q, c->soa, make_args<float>(c, c->pop[0], c->pop[0]), c->stream));
-            c->launches++;
+    int s = 0;
+    if (graph_wanted(c, n)) {
+        // the graph covers an even number of steps from a periodic state: get there first
+        if (c->fam == FAM_2POP && use_pull(c) && c->sto == STO_CANON && n > GRAPH_STEPS) {
+            if (int rc = one_step(c)) return rc;
+            ++s;
         }
-        c->steps++;
+        for (; n - s >= GRAPH_STEPS; s += GRAPH_STEPS) {
+            int rc = step_graphed(c);
+            if (rc == LBM_E_STATE) break;       // capture not possible here: fall back to plain launches
+            if (rc != LBM_OK) return rc;
+        }
     }
+    for (; s < n; ++s)
+        if (int rc = one_step(c)) return rc;
     return LBM_OK;
 }
+
+int lbm_set_graph(lbm_t* c, int mode)
+{
+    if (!c) { set_err("null context"); return LBM_E_ARG; }
+    if (mode != LBM_GRAPH_AUTO && mode != LBM_GRAPH_OFF && mode != LBM_GRAPH_ON) { set_err("unknown graph mode %d", mode); return LBM_E_ARG; }
+    c->graph_mode = mode;
+    drop_graph(c);
+    return LBM_OK;
+}
+long long lbm_graph_replays(const lbm_t* c) { return c ? c->graph_replays : -1; }
 
 int lbm_macroscopic_device(lbm_t* c, void* rho, void* u)
 {
@@ -444,7 +545,7 @@ int lbm_kinetic_energy(lbm_t* c, double* e)
     else
         CK(aux_energy<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr, load_mode(c)), c->partial,
                              c->n_partial, c->e_dev, c->stream));
-    c->launches += 2;
+    c->launches += 3;
     CK(cudaMemcpyAsync(e, c->e_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     return LBM_OK;
@@ -543,6 +644,7 @@ int lbm_set_block(lbm_t* c, int threads)
     if (!c) { set_err("null context"); return LBM_E_ARG; }
     if (threads < 32 || threads > 256 || (threads & 31)) { set_err("threads per block must be a multiple of 32 in [32, 256]"); return LBM_E_ARG; }
     c->block = threads;
+    drop_graph(c);
     return LBM_OK;
 }
 
@@ -554,6 +656,7 @@ int lbm_set_variant(lbm_t* c, int variant)
         if (int rc = normalise(c)) return rc;
     }
     c->variant = variant;
+    drop_graph(c);
     return LBM_OK;
 }
 

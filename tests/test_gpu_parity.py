@@ -171,3 +171,43 @@ def test_state_errors(Lbm):
     with pytest.raises(LbmError):
         Lbm(2, 8, 8)
     assert g.kernel_launches >= 1 and g.device_bytes > 0
+
+
+@pytest.mark.parametrize("scheme", ALL_SCHEMES)
+def test_graph_replay_is_bitwise_the_plain_path(Lbm, oracle, scheme):
+    """lbm_step through the captured CUDA graph (launch-bound lattices) == plain launches, bit for bit,
+    from even and odd starting parities, and both match the oracle"""
+    shape = (12, 9, 10)
+    chunks = [3, 40, 16, 1, 37, 3]          # graph blocks start at odd and even times
+    steps = sum(chunks)
+    g, o, fl = run_pair(Lbm, oracle, shape, 19, "BGK_W2", scheme, "f64", steps, kind="obstacle", chunks=chunks)
+    assert g.graph_replays >= 4
+    fg = g.get_populations()
+    assert pop_error(g, o, fl, 19, oracle, False) <= TOL64
+    h = Lbm(*shape, lattice=19, collision="BGK_W2", scheme=scheme, omega=1.7, dtype="f64")
+    fl2, uw = box_flags(*shape, "obstacle")
+    rho, u = inputs.seeded_init(*shape, 0)
+    h.set_flags(fl2, uw)
+    h.set_graph("off")
+    h.init_equilibrium(rho, u)
+    h.step(steps)
+    assert h.graph_replays == 0
+    assert np.array_equal(h.get_populations(), fg)
+    assert h.kernel_launches - 1 <= g.kernel_launches  # the graph's launches are counted too
+
+
+def test_graph_dropped_when_rates_change(Lbm, oracle):
+    """a setter between two lbm_step calls must not leave a stale graph behind"""
+    shape = (10, 10, 10)
+    fl, uw = box_flags(*shape, "cavity")
+    rho, u = inputs.seeded_init(*shape, 3)
+    g = Lbm(*shape, lattice=19, collision="RM", scheme="AA_SOA", omega=1.6, dtype="f64")
+    o = oracle.Oracle(*shape, Q=19, model="RM", omega=1.6)
+    for s in (g, o):
+        s.set_flags(fl, uw)
+        s.init_equilibrium(rho, u)
+        s.step(32)
+        s.set_relaxation(1.0, 1.2, 0.8)
+        s.step(33)
+    assert g.graph_replays >= 3
+    assert pop_error(g, o, fl, 19, oracle, False) <= TOL64
