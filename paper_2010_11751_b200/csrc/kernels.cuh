@@ -232,7 +232,7 @@ __global__ void __launch_bounds__(256, min_blocks<T, Q>()) step_kernel(const Ste
 #define LBM_MINB_SWAP_D27 2
 #endif
 template <class T, int Q, bool SOA>
-__global__ void __launch_bounds__(256, (Q == 27 && sizeof(T) == 8) ? LBM_MINB_SWAP_D27 : LBM_MINB_SWAP) swap_stream_kernel(const StepArgs<T> a)
+__global__ void __launch_bounds__(256, Q == 27 ? LBM_MINB_SWAP_D27 : LBM_MINB_SWAP) swap_stream_kernel(const StepArgs<T> a)
 {
     using L = Lat<Q>;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;

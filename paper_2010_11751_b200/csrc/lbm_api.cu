@@ -66,6 +66,8 @@ struct lbm_ctx {
     // CUDA-graph replay of lbm_step for launch-bound lattices (see step_graphed)
     int graph_mode;             // LBM_GRAPH_AUTO / OFF / ON
     cudaGraphExec_t graph_exec; // GRAPH_STEPS steps starting from graph_sto with pop[0] == graph_pop0
+    cudaStream_t cap_stream;    // private stream the capture runs on (the context stream may be the
+                                // legacy default stream, which cannot be captured); nothing executes on it
     Storage graph_sto;
     void* graph_pop0;
     long long graph_replays;
@@ -271,18 +273,27 @@ int step_graphed(lbm_ctx* c)
     if (c->graph_exec && (c->graph_sto != c->sto || c->graph_pop0 != c->pop[0])) drop_graph(c);
     if (!c->graph_exec) {
         cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
-        if (cudaStreamIsCapturing(c->stream, &st) != cudaSuccess || st != cudaStreamCaptureStatusNone) {
+        if (c->stream != nullptr && c->stream != cudaStreamLegacy && c->stream != cudaStreamPerThread &&
+            (cudaStreamIsCapturing(c->stream, &st) != cudaSuccess || st != cudaStreamCaptureStatusNone)) {
             cudaGetLastError();
             return LBM_E_STATE;  // the caller is capturing this stream itself
+        }
+        if (!c->cap_stream && cudaStreamCreateWithFlags(&c->cap_stream, cudaStreamNonBlocking) != cudaSuccess) {
+            c->cap_stream = nullptr;
+            cudaGetLastError();
+            return LBM_E_STATE;
         }
         const Storage sto0 = c->sto;
         void* const pop0 = c->pop[0];
         const long long steps0 = c->steps, launches0 = c->launches;
-        if (cudaStreamBeginCapture(c->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return LBM_E_STATE; }
+        cudaStream_t const user_stream = c->stream;
+        if (cudaStreamBeginCapture(c->cap_stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaGetLastError(); return LBM_E_STATE; }
+        c->stream = c->cap_stream;
         int rc = LBM_OK;
         for (int s = 0; s < GRAPH_STEPS && rc == LBM_OK; ++s) rc = one_step(c);
+        c->stream = user_stream;
         cudaGraph_t graph = nullptr;
-        cudaError_t e = cudaStreamEndCapture(c->stream, &graph);
+        cudaError_t e = cudaStreamEndCapture(c->cap_stream, &graph);
         // nothing ran: undo the bookkeeping of the captured steps
         c->steps = steps0; c->launches = launches0;
         const bool periodic = c->sto == sto0 && c->pop[0] == pop0;
@@ -399,6 +410,7 @@ int lbm_destroy(lbm_t* c)
     if (!c) return LBM_OK;
     cudaStreamSynchronize(c->stream);
     drop_graph(c);
+    if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
     dev_free(c, c->pop[0]);
     dev_free(c, c->pop[1]);
     dev_free(c, c->code);
