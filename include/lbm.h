@@ -40,7 +40,9 @@ enum { LBM_BGK_W2 = 0, LBM_BGK_NW4, LBM_TRT, LBM_RM, LBM_HM, LBM_CM, LBM_CHM, LB
 /* memory-access schemes x layouts (Table 1) */
 enum { LBM_2POP_SOA = 0, LBM_2POP_AOS, LBM_SWAP_SOA, LBM_SWAP_AOS, LBM_AA_SOA, LBM_AA_AOS, LBM_NUM_SCHEMES };
 enum { LBM_F32 = 0, LBM_F64 = 1 };
-enum { LBM_FLUID = 0, LBM_WALL = 1, LBM_MOVING = 2 }; /* cell flags */
+enum { LBM_FLUID = 0, LBM_WALL = 1, LBM_MOVING = 2, LBM_GHOST = 3 }; /* cell flags; LBM_GHOST = a
+   fluid cell owned by another rank of a slab decomposition: never updated and left out of every
+   sum and export, read like a fluid cell by its neighbours, filled by lbm_halo_unpack */
 enum { LBM_OK = 0, LBM_E_ARG = -1, LBM_E_ALLOC = -2, LBM_E_CUDA = -3, LBM_E_STATE = -4 };
 
 /* Device-memory and stream hooks (process-wide; set before lbm_create).  alloc returns a device
@@ -118,6 +120,24 @@ int lbm_set_variant(lbm_t* ctx, int variant);
 /* Threads per block of the step kernels (tuning knob of the sweep; multiple of 32 in [32, 256];
  * default 128).  Results do not depend on it. */
 int lbm_set_block(lbm_t* ctx, int threads);
+
+/* Halo exchange of a slab decomposition along x (the slowest axis: an x-layer is ny*nz contiguous
+ * cells of every SoA plane).  The paper's scheme is single-device; cells are
+ * coupled only through the one-cell stencil of Eq 2, so a rank owns the layers
+ * x = 1 .. nx-2 of its context and flags x = 0 and x = nx-1 LBM_GHOST (or WALL/MOVING where the
+ * neighbouring rank's layer is solid).  After every lbm_step(1):
+ *   lbm_halo_pack(face, buf)    buf <- post-collision populations of the owned layer next to the
+ *                               face that leave through it: face 0 (low x): cx = -1 of layer 1;
+ *                               face 1 (high x): cx = +1 of layer nx-2;
+ *   (send buf to that neighbour; receive its buffer of the opposite face)
+ *   lbm_halo_unpack(face, buf)  ghost layer of the face <- buf (face 0: cx = +1 into layer 0;
+ *                               face 1: cx = -1 into layer nx-1).
+ * buf is DEVICE memory of lbm_halo_count() elements of the context dtype, layout [dir][ny*nz] with
+ * directions in increasing k; asynchronous on the stream.  Two-population SoA scheme only
+ * (LBM_E_ARG otherwise); raw stored values, so both ranks must use the same dtype. */
+long long lbm_halo_count(const lbm_t* ctx);
+int lbm_halo_pack(lbm_t* ctx, int face, void* buf_dev);
+int lbm_halo_unpack(lbm_t* ctx, int face, const void* buf_dev);
 
 /* CUDA-graph replay of lbm_step.  A step of a lattice below ~96^3 cells lasts a few microseconds
  * and is bound by launch latency (the paper's "one synchronisation per step");

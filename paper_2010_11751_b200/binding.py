@@ -20,14 +20,14 @@ SCHEMES = {"2POP_SOA": 0, "2POP_AOS": 1, "SWAP_SOA": 2, "SWAP_AOS": 3, "AA_SOA":
 DTYPES = {"f32": 0, "f64": 1}
 NP_DTYPES = {"f32": np.float32, "f64": np.float64}
 VARIANTS = {"default": 0, "generic_push": 1, "generic_pull": 2}
-FLUID, WALL, MOVING = 0, 1, 2
+FLUID, WALL, MOVING, GHOST = 0, 1, 2, 3
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = [
     "lbm_set_hooks", "lbm_create", "lbm_destroy", "lbm_set_flags", "lbm_set_relaxation", "lbm_set_trt_magic",
     "lbm_init_equilibrium", "lbm_init_equilibrium_device", "lbm_step", "lbm_macroscopic", "lbm_macroscopic_device", "lbm_kinetic_energy", "lbm_get_populations", "lbm_get_populations_at",
     "lbm_set_populations", "lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches",
-    "lbm_sync", "lbm_set_variant", "lbm_set_block", "lbm_set_graph", "lbm_graph_replays", "lbm_last_error", "lbm_version",
+    "lbm_sync", "lbm_set_variant", "lbm_set_block", "lbm_set_graph", "lbm_graph_replays", "lbm_halo_count", "lbm_halo_pack", "lbm_halo_unpack", "lbm_last_error", "lbm_version",
 ]
 GRAPH_MODES = {"auto": 0, "off": 1, "on": 2}
 
@@ -70,6 +70,10 @@ def load_library(path=LIB_PATH):
     L.lbm_get_populations_at.argtypes = [vp, vp, i, vp]
     L.lbm_set_populations.argtypes = [vp, vp]
     L.lbm_set_graph.argtypes = [vp, i]
+    L.lbm_halo_count.restype = C.c_longlong
+    L.lbm_halo_count.argtypes = [vp]
+    L.lbm_halo_pack.argtypes = [vp, i, vp]
+    L.lbm_halo_unpack.argtypes = [vp, i, vp]
     for name in ("lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches", "lbm_graph_replays"):
         getattr(L, name).restype = C.c_longlong
         getattr(L, name).argtypes = [vp]
@@ -231,6 +235,17 @@ class Lbm:
     @property
     def kernel_launches(self):
         return self._L.lbm_kernel_launches(self._h)
+
+    @property
+    def halo_count(self):
+        """elements of one halo buffer (lbm_halo_pack / lbm_halo_unpack)"""
+        return self._L.lbm_halo_count(self._h)
+
+    def halo_pack(self, face, buf_ptr):
+        self._ck(self._L.lbm_halo_pack(self._h, int(face), C.c_void_p(buf_ptr)))
+
+    def halo_unpack(self, face, buf_ptr):
+        self._ck(self._L.lbm_halo_unpack(self._h, int(face), C.c_void_p(buf_ptr)))
 
     @property
     def graph_replays(self):

@@ -16,7 +16,7 @@ __global__ void classify_kernel(const uint8_t* __restrict__ flags, uint8_t* __re
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.n) return;
     const uint8_t fl = flags[i];
-    if (fl != 0) { code[i] = fl == 2 ? CODE_MOVING : CODE_WALL; mask[i] = 0ull; return; }
+    if (fl != 0) { code[i] = fl == 2 ? CODE_MOVING : fl == 3 ? CODE_GHOST : CODE_WALL; mask[i] = 0ull; return; }
     const int z = i % g.nz, y = (i / g.nz) % g.ny, x = i / (g.nz * g.ny);
     unsigned long long m = 0ull;
     if (x == 0) m |= 1ull << (MASK_FACE_SHIFT + 0);
@@ -30,7 +30,7 @@ __global__ void classify_kernel(const uint8_t* __restrict__ flags, uint8_t* __re
         if constexpr (k != L::REST) {
             const int n = (wrap1(x + L::cx(k), g.nx) * g.ny + wrap1(y + L::cy(k), g.ny)) * g.nz + wrap1(z + L::cz(k), g.nz);
             const uint8_t nf = flags[n];
-            if (nf != 0) m |= 1ull << link_of<Q>(k);
+            if (nf == 1 || nf == 2) m |= 1ull << link_of<Q>(k);  // a ghost neighbour (3) is read like a fluid one
             if (nf == 2) m |= 1ull << (MASK_MOVING_SHIFT + link_of<Q>(k));
         }
     });
@@ -184,6 +184,15 @@ cudaError_t aux_stream_only(int Q, bool soa, const StepArgs<T>& a, cudaStream_t 
     return cudaGetLastError();
 }
 
+template <class T>
+cudaError_t aux_halo(bool pack, T* pop, long long stride, const HaloArgs& p, T* buf, cudaStream_t s)
+{
+    const dim3 grid((p.cells + 255) / 256, p.ndir);
+    if (pack) halo_kernel<T, true><<<grid, 256, 0, s>>>(pop, stride, p, buf);
+    else halo_kernel<T, false><<<grid, 256, 0, s>>>(pop, stride, p, buf);
+    return cudaGetLastError();
+}
+
 #define LBM_AUX_INST(T)                                                                                                  \
     template cudaError_t aux_init_equilibrium<T>(int, bool, bool, T*, const uint8_t*, const Geo&, const T*, const T*,   \
                                                  cudaStream_t);                                                         \
@@ -193,6 +202,7 @@ cudaError_t aux_stream_only(int Q, bool soa, const StepArgs<T>& a, cudaStream_t 
                                               const int*, int, cudaStream_t);                                                           \
     template cudaError_t aux_insert_plane<T>(int, bool, T*, const uint8_t*, const Geo&, int, double, const T*,          \
                                              cudaStream_t);                                                             \
+    template cudaError_t aux_halo<T>(bool, T*, long long, const HaloArgs&, T*, cudaStream_t);                           \
     template cudaError_t aux_swap_stream<T>(int, bool, const StepArgs<T>&, cudaStream_t);                               \
     template cudaError_t aux_stream_only<T>(int, bool, const StepArgs<T>&, cudaStream_t);
 LBM_AUX_INST(float)

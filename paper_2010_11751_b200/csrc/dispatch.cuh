@@ -47,6 +47,8 @@ cudaError_t aux_insert_plane(int Q, bool soa, T* pop, const uint8_t* code, const
                              const T* in, cudaStream_t s);
 template <class T>
 cudaError_t aux_swap_stream(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s);
+template <class T>
+cudaError_t aux_halo(bool pack, T* pop, long long stride, const HaloArgs& p, T* buf, cudaStream_t s);
 // stream only (LD_PULL -> ST_LOCAL without collision): turns post-collision storage into canonical
 template <class T>
 cudaError_t aux_stream_only(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s);

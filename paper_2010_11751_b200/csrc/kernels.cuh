@@ -21,7 +21,9 @@
 // least one masked lane runs the masked path for all its lanes (selects on mask bits, no
 // divergence, no integer division).  Both give the same values for bulk cells.
 //
-// cell code byte: 0 = bulk fluid, 1 = wall, 2 = moving wall, 4 = fluid with a non-zero link mask.
+// cell code byte: 0 = bulk fluid, 1 = wall, 2 = moving wall, 3 = ghost (a fluid cell that another
+// rank owns: never updated here, read like a fluid cell by its neighbours, filled by
+// halo_unpack), 4 = fluid with a non-zero link mask.
 #pragma once
 #include "collision.cuh"
 
@@ -29,7 +31,7 @@ namespace lbm {
 
 enum { LD_LOCAL = 0, LD_PULL, LD_AAPULL };
 enum { ST_LOCAL = 0, ST_SWAPPED, ST_PUSH };
-enum { CODE_BULK = 0, CODE_WALL = 1, CODE_MOVING = 2, CODE_EDGE = 4 };
+enum { CODE_BULK = 0, CODE_WALL = 1, CODE_MOVING = 2, CODE_GHOST = 3, CODE_EDGE = 4 };
 enum { MASK_MOVING_SHIFT = 26, MASK_FACE_SHIFT = 52 };
 
 struct Geo {
@@ -395,7 +397,7 @@ __global__ void extract_plane_kernel(const T* __restrict__ pop, const uint8_t* _
             n = (wrap1(x - p.sx, g.nx) * g.ny + wrap1(y - p.sy, g.ny)) * g.nz + wrap1(z - p.sz, g.nz);
         }
         const int nc = code[n] & 3;
-        if (nc == 0) v = pop[slot<SOA, Q>(g, p.slot_fluid, n)];
+        if (nc == 0 || nc == CODE_GHOST) v = pop[slot<SOA, Q>(g, p.slot_fluid, n)];
         else v = pop[slot<SOA, Q>(g, p.slot_wall, i)] + (nc == CODE_MOVING ? T(p.wterm) : T(0));
         if (SHIFT) v += T(p.weight);
     }
@@ -411,6 +413,27 @@ __global__ void insert_plane_kernel(T* __restrict__ pop, const uint8_t* __restri
     T v = T(0);
     if (!(code[i] & 3)) v = SHIFT ? in[i] - T(weight) : in[i];
     pop[slot<SOA, Q>(g, k, i)] = v;
+}
+
+// halo exchange of the slab decomposition along x: one x-layer (ny*nz contiguous
+// cells in SoA) of the `ndir` population planes listed in p.dir, to (PACK) or from a contiguous
+// buffer [ndir][ny*nz].  Raw stored values (fp32: shifted), so both ends must have the same dtype.
+struct HaloArgs {
+    int dir[9];
+    int ndir;
+    long long first;   // index of the first cell of the layer
+    int cells;         // ny*nz
+};
+template <class T, bool PACK>
+__global__ void halo_kernel(T* __restrict__ pop, long long stride, HaloArgs p, T* __restrict__ buf)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= p.cells) return;
+    const int d = blockIdx.y;
+    T* slot = pop + (long long)p.dir[d] * stride + p.first + t;
+    T* b = buf + (long long)d * p.cells + t;
+    if (PACK) *b = *slot;
+    else *slot = *b;
 }
 
 }  // namespace lbm

@@ -426,7 +426,7 @@ int lbm_set_flags(lbm_t* c, const uint8_t* flags, const double u_wall[3])
     if (!c || !flags) { set_err("null argument"); return LBM_E_ARG; }
     long long nfluid = 0;
     for (int i = 0; i < c->g.n; ++i) {
-        if (flags[i] > LBM_MOVING) { set_err("flag %d at cell %d is not FLUID/WALL/MOVING", flags[i], i); return LBM_E_ARG; }
+        if (flags[i] > LBM_GHOST) { set_err("flag %d at cell %d is not FLUID/WALL/MOVING/GHOST", flags[i], i); return LBM_E_ARG; }
         nfluid += flags[i] == LBM_FLUID;
     }
     drop_graph(c);
@@ -636,6 +636,54 @@ int lbm_set_populations(lbm_t* c, const void* f)
     }
     CK(cudaStreamSynchronize(c->stream));
     c->sto = STO_CANON;
+    return LBM_OK;
+}
+
+// ---- halo exchange of the slab decomposition along x
+static int halo_check(lbm_t* c, int face, const void* buf)
+{
+    if (!c || !buf) { set_err("null argument"); return LBM_E_ARG; }
+    if (face != 0 && face != 1) { set_err("face must be 0 (low x) or 1 (high x)"); return LBM_E_ARG; }
+    if (c->scheme != LBM_2POP_SOA || !use_pull(c)) {
+        set_err("halo exchange is implemented for the two-population SoA scheme (pull form) only");
+        return LBM_E_ARG;
+    }
+    if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
+    return LBM_OK;
+}
+static HaloArgs halo_args(const lbm_t* c, int want_cx, int x_layer)
+{
+    HaloArgs p;
+    p.ndir = 0;
+    for (int k = 0; k < c->Q; ++k)
+        if (c->c[k][0] == want_cx) p.dir[p.ndir++] = k;
+    p.cells = c->ny * c->nz;
+    p.first = (long long)x_layer * p.cells;
+    return p;
+}
+long long lbm_halo_count(const lbm_t* c)
+{
+    if (!c) return -1;
+    return (long long)(c->Q == 19 ? 5 : 9) * c->ny * c->nz;
+}
+int lbm_halo_pack(lbm_t* c, int face, void* buf)
+{
+    if (int rc = halo_check(c, face, buf)) return rc;
+    // populations that leave through the face: cx = -1 from the first owned layer (x = 1), cx = +1 from the last (x = nx-2)
+    const HaloArgs p = halo_args(c, face == 0 ? -1 : +1, face == 0 ? 1 : c->nx - 2);
+    if (c->dtype == LBM_F64) CK(aux_halo<double>(true, (double*)c->pop[0], c->g.stride, p, (double*)buf, c->stream));
+    else CK(aux_halo<float>(true, (float*)c->pop[0], c->g.stride, p, (float*)buf, c->stream));
+    c->launches++;
+    return LBM_OK;
+}
+int lbm_halo_unpack(lbm_t* c, int face, const void* buf)
+{
+    if (int rc = halo_check(c, face, buf)) return rc;
+    // populations that enter through the face: cx = +1 into the low ghost layer (x = 0), cx = -1 into the high one (x = nx-1)
+    const HaloArgs p = halo_args(c, face == 0 ? +1 : -1, face == 0 ? 0 : c->nx - 1);
+    if (c->dtype == LBM_F64) CK(aux_halo<double>(false, (double*)c->pop[0], c->g.stride, p, (double*)buf, c->stream));
+    else CK(aux_halo<float>(false, (float*)c->pop[0], c->g.stride, p, (float*)buf, c->stream));
+    c->launches++;
     return LBM_OK;
 }
 

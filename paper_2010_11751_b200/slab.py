@@ -1,0 +1,196 @@
+"""Slab decomposition along x with a one-cell halo (the paper itself is single-device,
+PAPER.md:L122).
+
+Cells are coupled only through the one-cell stencil of Eq 2, so the lattice is cut
+into slabs of x-layers (x is the slowest axis: a layer is ny*nz contiguous cells of every SoA plane).
+Rank r owns the global layers [x0, x1) and runs an ordinary context of nx = (x1 - x0) + 2 layers whose
+first and last layer stand for the neighbours' nearest layers: LBM_GHOST where that layer is fluid
+(read like fluid, never updated, filled by the halo exchange), WALL / MOVING where it is solid (so
+bounce-back at a wall owned by another rank needs no communication).  The ranks form a ring, which is
+the periodic wrap of the library's index arithmetic; a cavity simply has walls at both ends of it.
+
+After every time step each rank sends, per face, the post-collision populations that leave through
+it (5 of 19 planes, 9 of 27) and receives the ones that enter: `lbm_halo_pack` -> send/recv ->
+`lbm_halo_unpack` (include/lbm.h).  That exchange is the only data-path communication; the kinetic
+energy adds one scalar all-reduce.  Two-population SoA scheme (pull form) only.
+
+This module holds the decomposition arithmetic and the exchange plumbing, no arithmetic of the
+method.  `exchange_local` serves several slabs living in one process (how the 1-GPU tests check the
+halo kernels against the oracle); `exchange_dist` is the one-process-per-GPU path over
+torch.distributed (NCCL on GPUs; the same code runs over gloo with CPU buffers in the host tests).
+"""
+import numpy as np
+
+FLUID, WALL, MOVING, GHOST = 0, 1, 2, 3
+
+
+def slab_range(NX, rank, world):
+    """global x-range [x0, x1) owned by `rank`: layers dealt as evenly as possible, low ranks first"""
+    if not (0 <= rank < world):
+        raise ValueError("rank %d outside [0, %d)" % (rank, world))
+    if NX < world:
+        raise ValueError("cannot cut %d layers into %d slabs" % (NX, world))
+    base, rem = divmod(NX, world)
+    x0 = rank * base + min(rank, rem)
+    return x0, x0 + base + (1 if rank < rem else 0)
+
+
+def neighbours(rank, world):
+    """(rank owning the layers below x0, rank owning the layers above x1) on the periodic ring"""
+    return (rank - 1) % world, (rank + 1) % world
+
+
+def _ghost_layer(layer):
+    return np.where(layer == FLUID, GHOST, layer).astype(np.uint8)
+
+
+def local_flags(flags, x0, x1):
+    """uint8 [x1-x0+2, ny, nz] from global flags [NX, ny, nz]: the owned layers between the two
+    neighbouring layers, where fluid becomes GHOST and solid stays solid"""
+    NX = flags.shape[0]
+    lo, hi = flags[(x0 - 1) % NX], flags[x1 % NX]
+    return np.concatenate([_ghost_layer(lo)[None], flags[x0:x1].astype(np.uint8), _ghost_layer(hi)[None]], axis=0)
+
+
+def local_field(a, x0, x1, axis=0):
+    """slice of a global field with one wrapped layer on either side along `axis` (the values in
+    the ghost layers are never used by the owner: its first step is local)"""
+    NX = a.shape[axis]
+    idx = np.arange(x0 - 1, x1 + 1) % NX
+    return np.ascontiguousarray(np.take(a, idx, axis=axis))
+
+
+def interior(a, axis=0):
+    """drop the two ghost layers of a local field"""
+    sl = [slice(None)] * a.ndim
+    sl[axis] = slice(1, -1)
+    return a[tuple(sl)]
+
+
+def exchange_local(engines):
+    """halo exchange between slabs that live in this process, engines[r] owning slab r of the ring.
+    An engine offers halo_pack(face) -> buffer and halo_unpack(face, buffer)."""
+    W = len(engines)
+    sent = [(e.halo_pack(0), e.halo_pack(1)) for e in engines]
+    for r, e in enumerate(engines):
+        left, right = neighbours(r, W)
+        e.halo_unpack(0, sent[left][1])    # what left the left neighbour through its high face
+        e.halo_unpack(1, sent[right][0])   # what left the right neighbour through its low face
+
+
+def exchange_dist(engine, dist, rank, world, group=None):
+    """the same over torch.distributed, one slab per process.  Buffers are torch tensors on the
+    backend's device (CUDA for nccl, CPU for gloo); the engine offers halo_pack(face) -> tensor,
+    halo_recv_buffer(face) -> tensor and halo_unpack(face, tensor)."""
+    s0, s1 = engine.halo_pack(0), engine.halo_pack(1)
+    r0, r1 = engine.halo_recv_buffer(0), engine.halo_recv_buffer(1)
+    if world == 1:
+        r0.copy_(s1)
+        r1.copy_(s0)
+    else:
+        left, right = neighbours(rank, world)
+        # the message tag is the face it LEFT through; nccl ignores tags and matches in order, so
+        # with two ranks (left == right) the receives are posted in the peer's send order
+        ops = [dist.P2POp(dist.isend, s0, left, group, 0), dist.P2POp(dist.isend, s1, right, group, 1),
+               dist.P2POp(dist.irecv, r1, right, group, 0), dist.P2POp(dist.irecv, r0, left, group, 1)]
+        for req in dist.batch_isend_irecv(ops):
+            req.wait()
+    engine.halo_unpack(0, r0)
+    engine.halo_unpack(1, r1)
+
+
+class GpuSlabEngine:
+    """one slab on the current CUDA device: an Lbm context plus its four halo buffers"""
+
+    def __init__(self, flags_local, u_wall, lattice=19, collision="BGK_W2", omega=1.0, dtype="f64"):
+        import torch
+        from .binding import Lbm, NP_DTYPES
+        nx, ny, nz = flags_local.shape
+        self.shape = (nx, ny, nz)
+        self.lbm = Lbm(nx, ny, nz, lattice=lattice, collision=collision, scheme="2POP_SOA", omega=omega, dtype=dtype)
+        self.lbm.set_flags(flags_local, u_wall)
+        tdt = torch.float64 if dtype == "f64" else torch.float32
+        self.np_dtype = NP_DTYPES[dtype]
+        cnt = self.lbm.halo_count
+        self._send = [torch.empty(cnt, dtype=tdt, device="cuda") for _ in range(2)]
+        self._recv = [torch.empty(cnt, dtype=tdt, device="cuda") for _ in range(2)]
+        self.halo_bytes = 2 * cnt * self._send[0].element_size()  # sent per step (received: the same)
+
+    def halo_pack(self, face):
+        self.lbm.halo_pack(face, self._send[face].data_ptr())
+        return self._send[face]
+
+    def halo_recv_buffer(self, face):
+        return self._recv[face]
+
+    def halo_unpack(self, face, buf):
+        self.lbm.halo_unpack(face, buf.data_ptr())
+
+    def close(self):
+        self.lbm.close()
+
+
+class SlabLbm:
+    """the user-facing multi-GPU object: one process per GPU, each owning one slab of an
+    NX x NY x NZ lattice.  `flags` / `rho` / `u` are GLOBAL host arrays (every rank passes the same
+    ones and keeps its slice); results come back per slab (macroscopic, populations) or global
+    (kinetic energy)."""
+
+    def __init__(self, NX, NY, NZ, flags=None, u_wall=(0.0, 0.0, 0.0), dist=None, rank=0, world=1, group=None,
+                 lattice=19, collision="BGK_W2", omega=1.0, dtype="f64"):
+        self.dist, self.rank, self.world, self.group = dist, rank, world, group
+        self.N = (NX, NY, NZ)
+        self.x0, self.x1 = slab_range(NX, rank, world)
+        if flags is None:
+            flags = np.zeros((NX, NY, NZ), dtype=np.uint8)
+        self.flags_local = local_flags(np.asarray(flags).reshape(NX, NY, NZ), self.x0, self.x1)
+        self.engine = GpuSlabEngine(self.flags_local, u_wall, lattice=lattice, collision=collision, omega=omega, dtype=dtype)
+        self.lbm = self.engine.lbm
+        self.Q = self.lbm.Q
+
+    def _local(self, a, lead):
+        NX, NY, NZ = self.N
+        a = np.asarray(a).reshape(lead + (NX, NY, NZ))
+        return local_field(a, self.x0, self.x1, axis=len(lead)).astype(self.engine.np_dtype)
+
+    def init_equilibrium(self, rho, u):
+        self.lbm.init_equilibrium(self._local(rho, ()), self._local(u, (3,)))
+
+    def exchange(self):
+        if self.dist is None or self.world == 1:
+            exchange_local([self.engine])
+        else:
+            exchange_dist(self.engine, self.dist, self.rank, self.world, self.group)
+
+    def step(self, n=1):
+        for _ in range(n):
+            self.lbm.step(1)
+            self.exchange()
+
+    def macroscopic(self):
+        """(rho [nxl, NY, NZ], u [3, nxl, NY, NZ]) of the owned layers"""
+        nx, ny, nz = self.engine.shape
+        rho, u = self.lbm.macroscopic()
+        return interior(rho.reshape(nx, ny, nz)).copy(), interior(u.reshape(3, nx, ny, nz), axis=1).copy()
+
+    def get_populations(self):
+        """f [Q, nxl, NY, NZ] of the owned layers, canonical order"""
+        nx, ny, nz = self.engine.shape
+        return interior(self.lbm.get_populations().reshape(self.Q, nx, ny, nz), axis=1).copy()
+
+    def kinetic_energy(self):
+        """global sum (one scalar all-reduce)"""
+        e = self.lbm.kinetic_energy()
+        if self.dist is not None and self.world > 1:
+            import torch
+            t = torch.tensor([e], dtype=torch.float64, device="cuda")
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
+            e = float(t.item())
+        return e
+
+    @property
+    def num_fluid(self):
+        return self.lbm.num_fluid
+
+    def close(self):
+        self.engine.close()

@@ -1,0 +1,210 @@
+"""Slab decomposition (paper_2010_11751_b200/slab.py): decomposition arithmetic, the exchange plumbing
+over gloo at world size 2 (CPU, with an oracle-backed engine standing in for the GPU context), and
+on the GPU several slabs in one process against the oracle's undivided lattice."""
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+from paper_2010_11751_b200 import inputs, slab
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_slab_range_covers_the_lattice():
+    for NX in (3, 7, 16, 257):
+        for world in (1, 2, 3, 5):
+            if NX < world:
+                continue
+            ranges = [slab.slab_range(NX, r, world) for r in range(world)]
+            assert ranges[0][0] == 0 and ranges[-1][1] == NX
+            for (a0, a1), (b0, b1) in zip(ranges, ranges[1:]):
+                assert a1 == b0
+            sizes = [b - a for a, b in ranges]
+            assert max(sizes) - min(sizes) <= 1 and min(sizes) >= 1
+    with pytest.raises(ValueError):
+        slab.slab_range(2, 0, 3)
+    assert slab.neighbours(0, 4) == (3, 1) and slab.neighbours(3, 4) == (2, 0) and slab.neighbours(0, 1) == (0, 0)
+
+
+def test_local_flags_ghost_and_solid_layers():
+    fl = inputs.cavity_flags(8, 5, 6)
+    lo = slab.local_flags(fl, 0, 4)        # below x0 = 0 lies the wall layer x = 7 (ring)
+    assert lo.shape == (6, 5, 6)
+    assert np.array_equal(lo[1:-1], fl[0:4])
+    assert np.array_equal(lo[0], fl[7])    # solid stays solid
+    inner = fl[4]
+    assert np.array_equal(lo[-1] == slab.GHOST, inner == slab.FLUID)
+    assert np.array_equal(lo[-1][inner != 0], inner[inner != 0])
+    a = np.arange(8 * 2).reshape(8, 2)
+    assert np.array_equal(slab.local_field(a, 0, 4)[:, 0], [14, 0, 2, 4, 6, 8])
+    assert np.array_equal(slab.interior(slab.local_field(a, 2, 5)), a[2:5])
+
+
+# ---------------------------------------------------------------- gloo, world size 2, CPU
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, %(root)r)
+import numpy as np, torch
+import torch.distributed as dist
+from paper_2010_11751_b200 import inputs, slab
+from oracle import lbm_oracle
+
+class OracleEngine:
+    # the oracle on one slab; ghost cells are plain fluid cells whose populations (all Q: the oracle
+    # collides them before it pushes) are overwritten by the exchange after every step
+    def __init__(self, flags_local, uw, Q, omega):
+        self.shape = flags_local.shape
+        nx, ny, nz = self.shape
+        self.Q = Q
+        self.o = lbm_oracle.Oracle(nx, ny, nz, Q=Q, model="BGK_W2", omega=omega)
+        self.o.set_flags(np.where(flags_local == slab.GHOST, 0, flags_local).astype(np.uint8), uw)
+        self.recv = [torch.empty(Q * ny * nz, dtype=torch.float64) for _ in range(2)]
+    def f(self):
+        return self.o.get_populations().reshape((self.Q,) + self.shape)
+    def halo_pack(self, face):
+        return torch.from_numpy(np.ascontiguousarray(self.f()[:, 1 if face == 0 else -2]).reshape(-1).copy())
+    def halo_recv_buffer(self, face):
+        return self.recv[face]
+    def halo_unpack(self, face, buf):
+        f = self.f().copy()
+        f[:, 0 if face == 0 else -1] = buf.numpy().reshape((self.Q,) + self.shape[1:])
+        self.o.set_populations(f.reshape(self.Q, -1))
+
+dist.init_process_group(backend="gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+NX, NY, NZ, Q, omega, steps = 9, 6, 5, %(Q)d, 1.7, 7
+for kind in ("cavity", "periodic"):
+    fl = inputs.cavity_flags(NX, NY, NZ) if kind == "cavity" else inputs.periodic_flags(NX, NY, NZ)
+    if kind == "periodic":
+        fl[4:6, 2:4, 1:3] = inputs.MOVING      # an obstacle that straddles the cut between the slabs
+    uw = (0.02, -0.01, 0.015)
+    rho, u = inputs.seeded_init(NX, NY, NZ, 1)
+    full = lbm_oracle.Oracle(NX, NY, NZ, Q=Q, model="BGK_W2", omega=omega)
+    full.set_flags(fl, uw); full.init_equilibrium(rho, u); full.step(steps)
+    x0, x1 = slab.slab_range(NX, rank, world)
+    e = OracleEngine(slab.local_flags(fl, x0, x1), uw, Q, omega)
+    e.o.init_equilibrium(slab.local_field(rho.reshape(NX, NY, NZ), x0, x1), slab.local_field(u.reshape(3, NX, NY, NZ), x0, x1, axis=1))
+    for _ in range(steps):
+        e.o.step(1)
+        slab.exchange_dist(e, dist, rank, world)
+    mine = slab.interior(e.f(), axis=1)
+    want = full.get_populations().reshape(Q, NX, NY, NZ)[:, x0:x1]
+    fluid = fl[x0:x1] == 0
+    err = np.abs(mine - want)[:, fluid].max()
+    assert err <= 1e-14, (kind, rank, err)
+dist.barrier()
+print("OK", rank)
+dist.destroy_process_group()
+"""
+
+
+@pytest.mark.parametrize("Q", [19, 27])
+def test_exchange_dist_gloo_world2(tmp_path, Q):
+    script = tmp_path / "w.py"
+    script.write_text(_WORKER % {"root": ROOT, "Q": Q})
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+           "--master-addr", "127.0.0.1", "--master-port", str(29530 + Q), str(script)]
+    r = subprocess.run(cmd, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stdout[-3000:] + r.stderr[-3000:]
+    assert r.stdout.count("OK") == 2
+
+
+# ---------------------------------------------------------------- GPU: several slabs in one process
+def _flags(kind, NX, NY, NZ):
+    if kind == "cavity":
+        return inputs.cavity_flags(NX, NY, NZ), (inputs.U_LID, 0.0, 0.0)
+    fl = inputs.periodic_flags(NX, NY, NZ)
+    fl[3:6, 2:4, 1:3] = inputs.MOVING
+    fl[NX - 1, 0:2, NZ // 2] = inputs.WALL
+    return fl, (0.01, -0.02, 0.015)
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("Q,dtype", [(19, "f64"), (27, "f64"), (19, "f32")])
+@pytest.mark.parametrize("kind", ["cavity", "obstacle"])
+@pytest.mark.parametrize("world", [1, 2, 3])
+def test_slabs_match_the_undivided_oracle(oracle, Q, dtype, kind, world):
+    NX, NY, NZ, omega, steps = 10, 9, 8, 1.7, 9
+    fl, uw = _flags(kind, NX, NY, NZ)
+    rho, u = inputs.seeded_init(NX, NY, NZ, 2)
+    npdt = np.float64 if dtype == "f64" else np.float32
+    rho, u = rho.astype(npdt), u.astype(npdt)
+    o = oracle.Oracle(NX, NY, NZ, Q=Q, model="BGK_W2", omega=omega)
+    o.set_flags(fl, uw)
+    o.init_equilibrium(rho.astype(np.float64), u.astype(np.float64))
+    o.step(steps)
+    want = o.get_populations().reshape(Q, NX, NY, NZ)
+    engines, ranges = [], []
+    for r in range(world):
+        x0, x1 = slab.slab_range(NX, r, world)
+        e = slab.GpuSlabEngine(slab.local_flags(fl, x0, x1), uw, lattice=Q, omega=omega, dtype=dtype)
+        e.lbm.init_equilibrium(slab.local_field(rho.reshape(NX, NY, NZ), x0, x1),
+                               slab.local_field(u.reshape(3, NX, NY, NZ), x0, x1, axis=1))
+        engines.append(e)
+        ranges.append((x0, x1))
+    for _ in range(steps):
+        for e in engines:
+            e.lbm.step(1)
+        slab.exchange_local(engines)
+    energy, nfluid = 0.0, 0
+    _, t, _, _ = oracle.lattice(Q)
+    for e, (x0, x1) in zip(engines, ranges):
+        nx = x1 - x0 + 2
+        got = slab.interior(e.lbm.get_populations().astype(np.float64).reshape(Q, nx, NY, NZ), axis=1)
+        fluid = fl[x0:x1] == 0
+        d = np.abs(got - want[:, x0:x1])[:, fluid]
+        if dtype == "f64":
+            assert d.max() <= 1e-12
+        else:
+            den = np.maximum(np.abs(want[:, x0:x1])[:, fluid], t[:, None])
+            assert (d / den).max() <= 2e-5
+        assert np.all(got[:, ~fluid] == 0.0)
+        energy += e.lbm.kinetic_energy()
+        nfluid += e.lbm.num_fluid
+        rho_l, u_l = e.lbm.macroscopic()
+        assert np.all(rho_l.reshape(nx, NY, NZ)[[0, -1]] == 0.0)   # ghost layers are left out of exports
+    assert nfluid == int((fl == 0).sum())
+    assert abs(energy - o.kinetic_energy()) <= (1e-12 if dtype == "f64" else 1e-6) * max(1.0, o.kinetic_energy())
+    for e in engines:
+        e.close()
+
+
+@pytest.mark.gpu
+def test_slab_lbm_single_rank_ring(oracle):
+    """SlabLbm at world size 1: the ring closes on itself, i.e. a periodic lattice in x"""
+    NX, NY, NZ, omega, steps = 8, 7, 9, 1.6, 6
+    fl = inputs.periodic_flags(NX, NY, NZ)
+    fl[:, 0, :] = inputs.WALL
+    rho, u = inputs.seeded_init(NX, NY, NZ, 5)
+    o = oracle.Oracle(NX, NY, NZ, Q=19, model="BGK_W2", omega=omega)
+    o.set_flags(fl, (0, 0, 0))
+    o.init_equilibrium(rho, u)
+    o.step(steps)
+    s = slab.SlabLbm(NX, NY, NZ, flags=fl, omega=omega)
+    s.init_equilibrium(rho, u)
+    s.step(steps)
+    got = s.get_populations()
+    want = o.get_populations().reshape(19, NX, NY, NZ)
+    assert np.abs(got - want)[:, fl == 0].max() <= 1e-12
+    assert abs(s.kinetic_energy() - o.kinetic_energy()) <= 1e-12
+    r, uu = s.macroscopic()
+    ro, uo = o.macroscopic()
+    assert np.abs(r - ro.reshape(NX, NY, NZ)).max() <= 1e-12 and np.abs(uu - uo.reshape(3, NX, NY, NZ)).max() <= 1e-12
+    s.close()
+
+
+@pytest.mark.gpu
+def test_halo_api_rejects_other_schemes():
+    import torch
+    from paper_2010_11751_b200 import Lbm
+    from paper_2010_11751_b200.binding import LbmError
+    g = Lbm(8, 8, 8, scheme="AA_SOA")
+    rho, u = inputs.seeded_init(8, 8, 8, 0)
+    g.init_equilibrium(rho, u)
+    buf = torch.empty(g.halo_count, dtype=torch.float64, device="cuda")
+    with pytest.raises(LbmError):
+        g.halo_pack(0, buf.data_ptr())
+    g.close()
