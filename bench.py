@@ -342,6 +342,95 @@ def run_gpu(args):
     print(json.dumps(line), flush=True)
 
 
+def run_gpu_slab(args):
+    """--decomp slab: ONE lattice of (N n) x n x n cells cut into N x-slabs, one per GPU, with a halo
+    exchange after every step (paper_2010_11751_b200/slab.py).  Weak scaling: every rank
+    owns n layers.  Two-population SoA workloads only."""
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the lattice Boltzmann path has no CPU fallback")
+    rank, world, dist = dist_setup(args.gpus)
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    from paper_2010_11751_b200 import slab
+    n, Q, model, scheme, dtype, re = WORKLOADS[args.workload]
+    if scheme != "2POP_SOA":
+        raise SystemExit("--decomp slab needs a two-population SoA workload (target2pop, 1)")
+    K, W = args.steps, max(args.warmup, 3)
+    NX = world * n
+    omega = inputs.omega_from_re(n, re)
+    x0, x1 = slab.slab_range(NX, rank, world)
+    fl, rho, u = slab.cavity_slab(NX, n, n, x0, x1, seed=0)
+    g = slab.SlabLbm(NX, n, n, flags_local=fl, u_wall=(inputs.U_LID, 0.0, 0.0), dist=dist, rank=rank, world=world,
+                     lattice=Q, collision=model, omega=omega, dtype=dtype)
+    nfluid = g.num_fluid
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    g.init_equilibrium_local(rho, u)
+    g.step(W)
+    sampler = ClockSampler(local_rank)
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    barrier()
+    sampler.start()
+    l0 = g.lbm.kernel_launches
+    e0.record()
+    g.step(K)
+    e1.record()
+    energy = g.kinetic_energy()
+    e2.record()
+    barrier()
+    launches = g.lbm.kernel_launches - l0
+    ms_steps, ms_total = e0.elapsed_time(e1), e0.elapsed_time(e2)
+    # end to end: host arrays in, K steps, host arrays out
+    barrier()
+    t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0.record()
+    g.init_equilibrium_local(rho, u)
+    g.step(K)
+    rho_out, u_out = g.macroscopic()
+    g.kinetic_energy()
+    t1.record()
+    barrier()
+    ms_e2e = t0.elapsed_time(t1)
+    clocks = sampler.stop()
+    assert np.isfinite(energy) and np.isfinite(rho_out).all()
+    ms_total_g, units_g = aggregate(dist, ms_total, nfluid * K, dev)
+    ms_e2e_g, _ = aggregate(dist, ms_e2e, 0, dev)
+    if rank != 0:
+        return
+    s = 8 if dtype == "f64" else 4
+    bpu = bytes_per_update(Q, dtype, scheme)
+    peak, peak_src = measured_peaks()
+    step_ms = ms_steps / K
+    achieved = nfluid * bpu / (step_ms * 1e-3) / 1e9
+    cfg = workload_config(args.workload, world)
+    cfg["workload"] = "%s, as ONE %d x %d x %d cavity cut into %d x-slabs" % (cfg["workload"], NX, n, n, world)
+    cfg["parallelism"] = "slab x%d along x, one-cell halo: %d of %d planes per face per step over torch.distributed p2p" % (
+        world, 5 if Q == 19 else 9, Q)
+    nloc = (x1 - x0 + 2) * n * n
+    line = {
+        "metric": METRIC, "value": units_g / (ms_total_g * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world, "steps": K,
+        "warmup": W, "ms_per_step": ms_total_g / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": dtype, "data": "synthetic", "config": cfg,
+        "roofline": {"bound": "hbm", "kernel": kernel_name(scheme, model, Q, dtype) + " + halo pack/unpack + exchange (rank 0)",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": traffic_from_profiles("target2pop", "step"), "peak_source": peak_src,
+                     "bytes_per_update": bpu, "updates_per_launch": nfluid, "ms_per_launch": step_ms},
+        "halo": {"bytes_sent_per_step_per_rank": g.engine.halo_bytes, "ms_per_step_incl_exchange": step_ms},
+        "e2e": {"value": units_g / (ms_e2e_g * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": 4 * nloc * s / K,
+                "d2h_bytes_per_step": (4 * nloc * s + 8) / K, "ms": ms_e2e_g,
+                "calls": "SlabLbm.init_equilibrium_local(host) -> step(K) -> macroscopic(host) + kinetic_energy"},
+        "gpu_launches": int(launches), "clocks": clocks, "fluid_cells": int(nfluid), "kinetic_energy": energy,
+    }
+    print(json.dumps(line), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -351,9 +440,13 @@ def main():
     ap.add_argument("--workload", default="target", choices=sorted(WORKLOADS))
     ap.add_argument("--variant", default=None, help="step-kernel variant (binding.VARIANTS), default = library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="replicas (default): N independent lattices; slab: one lattice cut along x with a halo exchange")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.decomp == "slab":
+        run_gpu_slab(args)
     else:
         run_gpu(args)
     try:

@@ -21,12 +21,13 @@ enum Variant {
     V_DEFAULT = 0,   // library's choice
     V_GENERIC_PUSH,  // generic one-thread-per-cell kernels, 2-pop as collide-then-push
     V_GENERIC_PULL,  // generic kernels, 2-pop as pull-then-collide with lazily streamed storage
+    V_AOS_PLAIN,     // AoS without the shared-memory tile (every access a per-thread gather / scatter)
     V_COUNT
 };
 
 // defined in inst.cu, explicitly instantiated once per (T, Q, MODEL)
 template <class T, int Q, int MODEL>
-cudaError_t launch_step(int kind, bool soa, int block, const StepArgs<T>& a, cudaStream_t s);
+cudaError_t launch_step(int kind, bool soa, int block, bool staged, const StepArgs<T>& a, cudaStream_t s);
 
 // defined in aux.cu
 cudaError_t aux_classify(int Q, const uint8_t* flags, uint8_t* code, unsigned long long* mask, const Geo& g, cudaStream_t s);

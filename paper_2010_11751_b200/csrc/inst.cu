@@ -9,31 +9,43 @@
 
 namespace lbm {
 
-template <class T, int Q, int MODEL, bool SOA>
-static cudaError_t launch_kind(int kind, int block, const StepArgs<T>& a, cudaStream_t s)
+template <class T, int Q, int MODEL, bool SOA, int LOAD, int STORE>
+static cudaError_t launch_one(int block, bool staged, const StepArgs<T>& a, cudaStream_t s)
 {
-    const int grid = (a.g.n + block - 1) / block;
-    switch (kind) {
-    case SK_PUSH: step_kernel<T, Q, MODEL, SOA, LD_LOCAL, ST_PUSH><<<grid, block, 0, s>>>(a); break;
-    case SK_PULL: step_kernel<T, Q, MODEL, SOA, LD_PULL, ST_LOCAL><<<grid, block, 0, s>>>(a); break;
-    case SK_COLLIDE: step_kernel<T, Q, MODEL, SOA, LD_LOCAL, ST_LOCAL><<<grid, block, 0, s>>>(a); break;
-    case SK_EVEN: step_kernel<T, Q, MODEL, SOA, LD_LOCAL, ST_SWAPPED><<<grid, block, 0, s>>>(a); break;
-    case SK_ODD: step_kernel<T, Q, MODEL, SOA, LD_AAPULL, ST_PUSH><<<grid, block, 0, s>>>(a); break;
-    default: return cudaErrorInvalidValue;
+    if constexpr (!SOA && (LOAD == LD_LOCAL || STORE != ST_PUSH)) {
+        if (staged) {  // AoS: local accesses through a transposing shared-memory tile (kernels.cuh)
+            const int b = block > 128 ? 128 : block;
+            step_kernel_aos<T, Q, MODEL, LOAD, STORE><<<(a.g.n + b - 1) / b, b, (size_t)b * Q * sizeof(T), s>>>(a);
+            return cudaGetLastError();
+        }
     }
+    step_kernel<T, Q, MODEL, SOA, LOAD, STORE><<<(a.g.n + block - 1) / block, block, 0, s>>>(a);
     return cudaGetLastError();
 }
 
-template <class T, int Q, int MODEL>
-cudaError_t launch_step(int kind, bool soa, int block, const StepArgs<T>& a, cudaStream_t s)
+template <class T, int Q, int MODEL, bool SOA>
+static cudaError_t launch_kind(int kind, int block, bool staged, const StepArgs<T>& a, cudaStream_t s)
 {
-    if (block <= 0 || block > 256 || (block & 31)) return cudaErrorInvalidValue;
-    return soa ? launch_kind<T, Q, MODEL, true>(kind, block, a, s) : launch_kind<T, Q, MODEL, false>(kind, block, a, s);
+    switch (kind) {
+    case SK_PUSH: return launch_one<T, Q, MODEL, SOA, LD_LOCAL, ST_PUSH>(block, staged, a, s);
+    case SK_PULL: return launch_one<T, Q, MODEL, SOA, LD_PULL, ST_LOCAL>(block, staged, a, s);
+    case SK_COLLIDE: return launch_one<T, Q, MODEL, SOA, LD_LOCAL, ST_LOCAL>(block, staged, a, s);
+    case SK_EVEN: return launch_one<T, Q, MODEL, SOA, LD_LOCAL, ST_SWAPPED>(block, staged, a, s);
+    case SK_ODD: return launch_one<T, Q, MODEL, SOA, LD_AAPULL, ST_PUSH>(block, staged, a, s);
+    default: return cudaErrorInvalidValue;
+    }
 }
 
-template cudaError_t launch_step<double, LBM_INST_Q, LBM_INST_MODEL>(int, bool, int, const StepArgs<double>&, cudaStream_t);
+template <class T, int Q, int MODEL>
+cudaError_t launch_step(int kind, bool soa, int block, bool staged, const StepArgs<T>& a, cudaStream_t s)
+{
+    if (block <= 0 || block > 256 || (block & 31)) return cudaErrorInvalidValue;
+    return soa ? launch_kind<T, Q, MODEL, true>(kind, block, staged, a, s) : launch_kind<T, Q, MODEL, false>(kind, block, staged, a, s);
+}
+
+template cudaError_t launch_step<double, LBM_INST_Q, LBM_INST_MODEL>(int, bool, int, bool, const StepArgs<double>&, cudaStream_t);
 #if LBM_INST_MODEL == 0 || LBM_INST_MODEL == 2 || LBM_INST_MODEL == 9
-template cudaError_t launch_step<float, LBM_INST_Q, LBM_INST_MODEL>(int, bool, int, const StepArgs<float>&, cudaStream_t);
+template cudaError_t launch_step<float, LBM_INST_Q, LBM_INST_MODEL>(int, bool, int, bool, const StepArgs<float>&, cudaStream_t);
 #endif
 
 }  // namespace lbm

@@ -235,6 +235,50 @@ __global__ void __launch_bounds__(256, min_blocks<T, Q>()) step_kernel(const Ste
     store_cell<T, Q, SOA, STORE>(a, i, cs.masked, cs.mask, f);
 }
 
+// AoS with shared-memory staging.  In the AoS layout pop[N][Q] the Q values of
+// the cells of one block are one contiguous run of blockDim*Q elements, but a warp that reads
+// "slot k of 32 consecutive cells" touches 32 different sectors.  Whatever is LOCAL to the cell
+// (the loads of 2-pop push / AA even / swap pass 1 / collide-only, the stores of 2-pop pull /
+// AA even / swap pass 1 / collide-only) therefore goes through a transposing tile: the block
+// copies its run coalesced, each thread works on its own record tile[tid*Q .. tid*Q+Q) (Q is odd,
+// so both 4-byte and 8-byte records are free of bank conflicts).  Neighbour accesses (LD_PULL,
+// LD_AAPULL, ST_PUSH) stay per-thread gathers / scatters.  Launch with blockDim*Q*sizeof(T) bytes
+// of dynamic shared memory.
+template <class T, int Q, int MODEL, int LOAD, int STORE>
+__global__ void __launch_bounds__(128) step_kernel_aos(const StepArgs<T> a)
+{
+    static_assert(LOAD == LD_LOCAL || STORE != ST_PUSH, "nothing to stage");
+    constexpr bool SHIFT = sizeof(T) == 4;
+    using L = Lat<Q>;
+    extern __shared__ __align__(16) unsigned char tile_raw[];
+    T* tile = reinterpret_cast<T*>(tile_raw);
+    const long long base = (long long)blockIdx.x * blockDim.x;   // first cell of the block
+    const int i = (int)base + threadIdx.x;
+    const int nb = min((long long)blockDim.x, (long long)a.g.n - base) * Q;   // elements of the block's run
+    const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
+    T* rec = tile + threadIdx.x * Q;
+    T f[Q];
+    if constexpr (LOAD == LD_LOCAL) {
+        const T* __restrict__ run = a.src + base * Q;
+        for (int e = threadIdx.x; e < nb; e += blockDim.x) tile[e] = run[e];
+        __syncthreads();
+        if (cs.active) static_for<Q>([&](auto kc) { f[kc] = rec[kc]; });
+    } else {
+        if (cs.active) load_cell<T, Q, false, LOAD>(a, i, cs.masked, cs.mask, f);
+        // the other array is written: solid cells of the run get zeros (never read)
+        if (!cs.active) static_for<Q>([&](auto kc) { rec[kc] = T(0); });
+    }
+    if (cs.active) collide<Q, MODEL, SHIFT>(f, a.rt);
+    if constexpr (STORE == ST_PUSH) {
+        if (cs.active) store_cell<T, Q, false, STORE>(a, i, cs.masked, cs.mask, f);
+    } else {
+        if (cs.active) static_for<Q>([&](auto kc) { rec[STORE == ST_SWAPPED ? L::opp(kc) : (int)kc] = f[kc]; });
+        __syncthreads();
+        T* __restrict__ run = a.dst + base * Q;
+        for (int e = threadIdx.x; e < nb; e += blockDim.x) run[e] = tile[e];
+    }
+}
+
 // ------------------------------------------------------------------ swap scheme, pass 2
 // After pass 1 pop_kbar(x) holds f_out_k(x).  For the half set k < NH (R5): exchange pop_kbar(x)
 // with pop_k(x + c_k) when that neighbour is fluid, else add w_k in place (the value already sits

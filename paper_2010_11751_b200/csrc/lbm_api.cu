@@ -152,23 +152,24 @@ template <class T, int Q>
 cudaError_t step_model(const lbm_ctx* c, int kind, const StepArgs<T>& a)
 {
     const bool soa = c->soa;
+    const bool st = c->variant != V_AOS_PLAIN;
     const int b = c->block;
     cudaStream_t s = c->stream;
     switch (c->model) {
-    case LBM_BGK_W2: return launch_step<T, Q, M_BGK_W2>(kind, soa, b, a, s);
-    case LBM_TRT: return launch_step<T, Q, M_TRT>(kind, soa, b, a, s);
-    case LBM_REG: return launch_step<T, Q, M_REG>(kind, soa, b, a, s);
+    case LBM_BGK_W2: return launch_step<T, Q, M_BGK_W2>(kind, soa, b, st, a, s);
+    case LBM_TRT: return launch_step<T, Q, M_TRT>(kind, soa, b, st, a, s);
+    case LBM_REG: return launch_step<T, Q, M_REG>(kind, soa, b, st, a, s);
     default: break;
     }
     if constexpr (sizeof(T) == 8) {
         switch (c->model) {
-        case LBM_BGK_NW4: return launch_step<T, Q, M_BGK_NW4>(kind, soa, b, a, s);
-        case LBM_RM: return launch_step<T, Q, M_RM>(kind, soa, b, a, s);
-        case LBM_HM: return launch_step<T, Q, M_HM>(kind, soa, b, a, s);
-        case LBM_CM: return launch_step<T, Q, M_CM>(kind, soa, b, a, s);
-        case LBM_CHM: return launch_step<T, Q, M_CHM>(kind, soa, b, a, s);
-        case LBM_K: return launch_step<T, Q, M_K>(kind, soa, b, a, s);
-        case LBM_RR: return launch_step<T, Q, M_RR>(kind, soa, b, a, s);
+        case LBM_BGK_NW4: return launch_step<T, Q, M_BGK_NW4>(kind, soa, b, st, a, s);
+        case LBM_RM: return launch_step<T, Q, M_RM>(kind, soa, b, st, a, s);
+        case LBM_HM: return launch_step<T, Q, M_HM>(kind, soa, b, st, a, s);
+        case LBM_CM: return launch_step<T, Q, M_CM>(kind, soa, b, st, a, s);
+        case LBM_CHM: return launch_step<T, Q, M_CHM>(kind, soa, b, st, a, s);
+        case LBM_K: return launch_step<T, Q, M_K>(kind, soa, b, st, a, s);
+        case LBM_RR: return launch_step<T, Q, M_RR>(kind, soa, b, st, a, s);
         default: break;
         }
     }

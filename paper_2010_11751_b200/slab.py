@@ -60,6 +60,20 @@ def local_field(a, x0, x1, axis=0):
     return np.ascontiguousarray(np.take(a, idx, axis=axis))
 
 
+def cavity_slab(NX, NY, NZ, x0, x1, seed=0):
+    """(flags_local, rho_local, u_local) of the slab [x0, x1) of an NX x NY x NZ lid-driven cavity with
+    the seeded noise init of inputs.py, built layer by layer so that no rank ever holds the global
+    arrays (weak-scaling runs); the values are those of the undivided lattice."""
+    from . import inputs
+    pattern = inputs.cavity_flags(3, NY, NZ)      # [0] = a wall layer, [1] = an inner layer
+    xs = np.arange(x0 - 1, x1 + 1) % NX
+    fl = np.stack([pattern[0] if (x == 0 or x == NX - 1) else pattern[1] for x in xs])
+    fl[0], fl[-1] = _ghost_layer(fl[0]), _ghost_layer(fl[-1])
+    cells = (xs.astype(np.int64)[:, None] * (NY * NZ) + np.arange(NY * NZ, dtype=np.int64)[None, :]).reshape(-1)
+    rho, u = inputs.seeded_init(len(xs), NY, NZ, seed, index_offset=cells)
+    return fl, rho, u
+
+
 def interior(a, axis=0):
     """drop the two ghost layers of a local field"""
     sl = [slice(None)] * a.ndim
@@ -137,13 +151,18 @@ class SlabLbm:
     (kinetic energy)."""
 
     def __init__(self, NX, NY, NZ, flags=None, u_wall=(0.0, 0.0, 0.0), dist=None, rank=0, world=1, group=None,
-                 lattice=19, collision="BGK_W2", omega=1.0, dtype="f64"):
+                 lattice=19, collision="BGK_W2", omega=1.0, dtype="f64", flags_local=None):
+        """flags: GLOBAL [NX, NY, NZ] (None = all fluid), or flags_local: this rank's [nxl+2, NY, NZ]
+        with its ghost layers already in place (local_flags / cavity_slab)"""
         self.dist, self.rank, self.world, self.group = dist, rank, world, group
         self.N = (NX, NY, NZ)
         self.x0, self.x1 = slab_range(NX, rank, world)
-        if flags is None:
-            flags = np.zeros((NX, NY, NZ), dtype=np.uint8)
-        self.flags_local = local_flags(np.asarray(flags).reshape(NX, NY, NZ), self.x0, self.x1)
+        if flags_local is not None:
+            self.flags_local = np.ascontiguousarray(flags_local, dtype=np.uint8).reshape(self.x1 - self.x0 + 2, NY, NZ)
+        else:
+            if flags is None:
+                flags = np.zeros((NX, NY, NZ), dtype=np.uint8)
+            self.flags_local = local_flags(np.asarray(flags).reshape(NX, NY, NZ), self.x0, self.x1)
         self.engine = GpuSlabEngine(self.flags_local, u_wall, lattice=lattice, collision=collision, omega=omega, dtype=dtype)
         self.lbm = self.engine.lbm
         self.Q = self.lbm.Q
@@ -155,6 +174,10 @@ class SlabLbm:
 
     def init_equilibrium(self, rho, u):
         self.lbm.init_equilibrium(self._local(rho, ()), self._local(u, (3,)))
+
+    def init_equilibrium_local(self, rho_local, u_local):
+        """rho [nxl+2, NY, NZ], u [3, nxl+2, NY, NZ] of this rank's context, ghost layers included"""
+        self.lbm.init_equilibrium(np.asarray(rho_local, dtype=self.engine.np_dtype), np.asarray(u_local, dtype=self.engine.np_dtype))
 
     def exchange(self):
         if self.dist is None or self.world == 1:

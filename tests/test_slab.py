@@ -43,6 +43,18 @@ def test_local_flags_ghost_and_solid_layers():
     assert np.array_equal(slab.interior(slab.local_field(a, 2, 5)), a[2:5])
 
 
+def test_cavity_slab_equals_slices_of_the_global_inputs():
+    NX, NY, NZ = 12, 5, 6
+    fl = inputs.cavity_flags(NX, NY, NZ)
+    rho, u = inputs.seeded_init(NX, NY, NZ, 4)
+    for rank in range(3):
+        x0, x1 = slab.slab_range(NX, rank, 3)
+        f, r, uu = slab.cavity_slab(NX, NY, NZ, x0, x1, seed=4)
+        assert np.array_equal(f, slab.local_flags(fl, x0, x1))
+        assert np.array_equal(r.reshape(-1, NY, NZ), slab.local_field(rho.reshape(NX, NY, NZ), x0, x1))
+        assert np.array_equal(uu.reshape(3, -1, NY, NZ), slab.local_field(u.reshape(3, NX, NY, NZ), x0, x1, axis=1))
+
+
 # ---------------------------------------------------------------- gloo, world size 2, CPU
 _WORKER = r"""
 import os, sys
