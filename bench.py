@@ -209,7 +209,9 @@ def workload_config(name, world):
                     % (name, Q, model, n, dtype, scheme, re),
         "lattice": "D3Q%d" % Q, "collision": model, "scheme": scheme, "n": n, "re": re,
         "parallelism": "replicas x%d (no data-path collective)" % world,
-        "l2": "populations %.2f GB per array >> 126 MB L2, no flush needed" % (n ** 3 * Q * (8 if dtype == "f64" else 4) / 1e9),
+        "l2": ("populations %.2f GB per array >> 126 MB L2, no flush needed" if n >= 128 else
+               "populations %.3f GB per array fit the 126 MB L2: launch-bound lattice, MLUPS reported, no HBM roofline claim")
+              % (n ** 3 * Q * (8 if dtype == "f64" else 4) / 1e9),
     }
 
 

@@ -57,7 +57,11 @@ struct StepArgs {
     //   sto[k]    where the pure store of f_k goes, in BYTES: ST_LOCAL plane[k]; ST_SWAPPED
     //             plane[kbar]; ST_PUSH plane[k] + off_k*IS                (times sizeof(T))
     // with IS = 1 (SoA) or Q (AoS) elements per cell step and off_k the cell-index offset of c_k.
-    long long plane[27], ldo[27], sto[27];
+    //   wlo[k]    byte offset of the slot the masked load of f_k reads when the upstream cell is
+    //             solid: LD_PULL plane[kbar]; LD_AAPULL plane[k]
+    //   wso[k]    byte offset of the slot the masked ST_PUSH store of f_k writes when the
+    //             downstream cell is solid: plane[kbar]
+    long long plane[27], ldo[27], sto[27], wlo[27], wso[27];
 };
 
 template <bool SOA, int Q>
@@ -79,40 +83,50 @@ __device__ __forceinline__ int offset(const Geo& g)
 template <int Q>
 __host__ __device__ constexpr int link_of(int k) { return k < Lat<Q>::REST ? k : k - 1; }
 
-// per-thread view of a link mask: wrapped index offsets to the six axis neighbours
+// per-thread view of a link mask
 struct Edge {
-    unsigned long long m;
-    int oxm, oxp, oym, oyp, ozm, ozp;
-    __device__ __forceinline__ Edge(unsigned long long mask, const Geo& g) : m(mask)
+    unsigned solid, moving, face;
+    // cell-index corrections that turn the plain neighbour offset into the periodically wrapped one
+    // (zero unless the cell lies on that face of the box)
+    int fxm, fxp, fym, fyp, fzm, fzp;
+    __device__ __forceinline__ Edge(unsigned long long mask, const Geo& g)
     {
+        solid = (unsigned)mask & ((1u << MASK_MOVING_SHIFT) - 1u);
+        moving = (unsigned)(mask >> MASK_MOVING_SHIFT) & ((1u << MASK_MOVING_SHIFT) - 1u);
+        face = (unsigned)(mask >> MASK_FACE_SHIFT);
         const int sx = g.ny * g.nz, sy = g.nz;
-        const unsigned f = (unsigned)(mask >> MASK_FACE_SHIFT);
-        oxm = (f & 1u) ? (g.nx - 1) * sx : -sx;
-        oxp = (f & 2u) ? -(g.nx - 1) * sx : sx;
-        oym = (f & 4u) ? (g.ny - 1) * sy : -sy;
-        oyp = (f & 8u) ? -(g.ny - 1) * sy : sy;
-        ozm = (f & 16u) ? (g.nz - 1) : -1;
-        ozp = (f & 32u) ? -(g.nz - 1) : 1;
+        fxm = (face & 1u) ? g.nx * sx : 0;
+        fxp = (face & 2u) ? -g.nx * sx : 0;
+        fym = (face & 4u) ? g.ny * sy : 0;
+        fyp = (face & 8u) ? -g.ny * sy : 0;
+        fzm = (face & 16u) ? g.nz : 0;
+        fzp = (face & 32u) ? -g.nz : 0;
     }
-    // index offset to the cell at x + SIGN * c_K, periodic wrap included
+    // wrap correction (in cells) of the neighbour at x + SIGN * c_K
     template <int Q, int K, int SIGN>
-    __device__ __forceinline__ int off() const
+    __device__ __forceinline__ int fix() const
     {
         using L = Lat<Q>;
         constexpr int dx = SIGN * L::cx(K), dy = SIGN * L::cy(K), dz = SIGN * L::cz(K);
         int o = 0;
-        if constexpr (dx == 1) o += oxp;
-        if constexpr (dx == -1) o += oxm;
-        if constexpr (dy == 1) o += oyp;
-        if constexpr (dy == -1) o += oym;
-        if constexpr (dz == 1) o += ozp;
-        if constexpr (dz == -1) o += ozm;
+        if constexpr (dx == 1) o += fxp;
+        if constexpr (dx == -1) o += fxm;
+        if constexpr (dy == 1) o += fyp;
+        if constexpr (dy == -1) o += fym;
+        if constexpr (dz == 1) o += fzp;
+        if constexpr (dz == -1) o += fzm;
         return o;
     }
+    // index offset to the cell at x + SIGN * c_K, periodic wrap included
+    template <int Q, int K, int SIGN>
+    __device__ __forceinline__ int off(const Geo& g) const
+    {
+        return SIGN * offset<Q, K>(g) + fix<Q, K, SIGN>();
+    }
     template <int Q, int K>
-    __device__ __forceinline__ bool solid() const { return (m >> link_of<Q>(K)) & 1ull; }
+    __device__ __forceinline__ bool solid_at() const { return (solid >> link_of<Q>(K)) & 1u; }
     template <int Q, int K>
-    __device__ __forceinline__ bool moving() const { return (m >> (MASK_MOVING_SHIFT + link_of<Q>(K))) & 1ull; }
+    __device__ __forceinline__ bool moving_at() const { return (moving >> link_of<Q>(K)) & 1u; }
 };
 
 // ------------------------------------------------------------------ load / store of one cell
@@ -128,18 +142,16 @@ __device__ __forceinline__ void load_cell(const StepArgs<T>& a, int i, bool mask
         static_for<Q>([&](auto kc) { f[kc] = *reinterpret_cast<const T*>(p + a.ldo[kc]); });
     } else {
         const Edge e(mask, a.g);
+        const char* __restrict__ p = reinterpret_cast<const char*>(src + (long long)i * IS);
         static_for<Q>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
             if constexpr (k == L::REST) {
-                f[k] = src[a.plane[k] + (long long)i * IS];
+                f[k] = *reinterpret_cast<const T*>(p + a.ldo[k]);
             } else {
-                // the upstream neighbour x - c_k = x + c_kbar
-                constexpr int s_fluid = LOAD == LD_PULL ? k : kb, s_wall = LOAD == LD_PULL ? kb : k;
-                const bool sol = e.template solid<Q, kb>();
-                const long long a_fluid = a.plane[s_fluid] + (long long)(i + e.template off<Q, k, -1>()) * IS;
-                const long long a_wall = a.plane[s_wall] + (long long)i * IS;
-                T v = src[sol ? a_wall : a_fluid];
-                if (e.template moving<Q, kb>()) v += a.wterm[kb];
+                // the upstream neighbour x - c_k = x + c_kbar: link kbar
+                const long long o_fluid = a.ldo[k] + (long long)e.template fix<Q, k, -1>() * (long long)(IS * sizeof(T));
+                T v = *reinterpret_cast<const T*>(p + (e.template solid_at<Q, kb>() ? a.wlo[k] : o_fluid));
+                if (e.template moving_at<Q, kb>()) v += a.wterm[kb];
                 f[k] = v;
             }
         });
@@ -157,17 +169,16 @@ __device__ __forceinline__ void store_cell(const StepArgs<T>& a, int i, bool mas
         static_for<Q>([&](auto kc) { *reinterpret_cast<T*>(p + a.sto[kc]) = f[kc]; });
     } else {
         const Edge e(mask, a.g);
+        char* __restrict__ p = reinterpret_cast<char*>(dst + (long long)i * IS);
         static_for<Q>([&](auto kc) {
-            constexpr int k = kc, kb = L::opp(k);
+            constexpr int k = kc;
             if constexpr (k == L::REST) {
-                dst[a.plane[k] + (long long)i * IS] = f[k];
+                *reinterpret_cast<T*>(p + a.sto[k]) = f[k];
             } else {
-                const bool sol = e.template solid<Q, k>();
-                const long long a_fluid = a.plane[k] + (long long)(i + e.template off<Q, k, +1>()) * IS;
-                const long long a_wall = a.plane[kb] + (long long)i * IS;
+                const long long o_fluid = a.sto[k] + (long long)e.template fix<Q, k, +1>() * (long long)(IS * sizeof(T));
                 T v = f[k];
-                if (e.template moving<Q, k>()) v += a.wterm[k];
-                dst[sol ? a_wall : a_fluid] = v;
+                if (e.template moving_at<Q, k>()) v += a.wterm[k];
+                *reinterpret_cast<T*>(p + (e.template solid_at<Q, k>() ? a.wso[k] : o_fluid)) = v;
             }
         });
     }
@@ -285,14 +296,12 @@ __global__ void __launch_bounds__(128) step_kernel_aos(const StepArgs<T> a)
 // in the slot Eq 3 sends it to); and when the neighbour at x - c_k is a wall, add w_kbar to pop_k(x).
 // Every slot is touched by exactly one thread (Table 1), so all loads
 // are issued before the first store.
-#ifndef LBM_MINB_SWAP
-#define LBM_MINB_SWAP 3
-#endif
-#ifndef LBM_MINB_SWAP_D27
-#define LBM_MINB_SWAP_D27 2
-#endif
+// resident blocks of 256 threads per SM for pass 2 (register cap), tuned on B200: fp64 3 / 2 (D3Q19 / D3Q27),
+// fp32 4 / 3.  Uncapped, the D3Q27 fp64 instance took 144 registers (one block per SM, 65 % of the copy rate).
+template <class T, int Q>
+constexpr int swap_min_blocks() { return (sizeof(T) == 8 ? 3 : 4) - (Q == 27 ? 1 : 0); }
 template <class T, int Q, bool SOA>
-__global__ void __launch_bounds__(256, Q == 27 ? LBM_MINB_SWAP_D27 : LBM_MINB_SWAP) swap_stream_kernel(const StepArgs<T> a)
+__global__ void __launch_bounds__(256, swap_min_blocks<T, Q>()) swap_stream_kernel(const StepArgs<T> a)
 {
     using L = Lat<Q>;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -319,25 +328,25 @@ __global__ void __launch_bounds__(256, Q == 27 ? LBM_MINB_SWAP_D27 : LBM_MINB_SW
         const Edge e(cs.mask, g);
         static_for<L::NH>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
-            const bool sol = e.template solid<Q, k>();
-            const long long pb = sol ? slot<SOA, Q>(g, k, i) : slot<SOA, Q>(g, k, (long long)i + e.template off<Q, k, +1>());
+            const bool sol = e.template solid_at<Q, k>();
+            const long long pb = sol ? slot<SOA, Q>(g, k, i) : slot<SOA, Q>(g, k, (long long)i + e.template off<Q, k, +1>(g));
             va[k] = pop[slot<SOA, Q>(g, kb, i)];
             vb[k] = pop[pb];
         });
         static_for<L::NH>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
-            const bool sol = e.template solid<Q, k>();
-            const bool back_moving = e.template moving<Q, kb>();   // neighbour at x - c_k
+            const bool sol = e.template solid_at<Q, k>();
+            const bool back_moving = e.template moving_at<Q, kb>();   // neighbour at x - c_k
             const long long pa = slot<SOA, Q>(g, kb, i);
             if (!sol) {
-                const long long pb = slot<SOA, Q>(g, k, (long long)i + e.template off<Q, k, +1>());
+                const long long pb = slot<SOA, Q>(g, k, (long long)i + e.template off<Q, k, +1>(g));
                 pop[pa] = vb[k];
                 pop[pb] = va[k];
                 // pop_k(x) belongs to the exchange of the cell at x - c_k unless that one is solid
                 if (back_moving) pop[slot<SOA, Q>(g, k, i)] += a.wterm[kb];
             } else {
                 // vb[k] holds pop_k(x) here
-                if (e.template moving<Q, k>()) pop[pa] = va[k] + a.wterm[k];
+                if (e.template moving_at<Q, k>()) pop[pa] = va[k] + a.wterm[k];
                 if (back_moving) pop[slot<SOA, Q>(g, k, i)] = vb[k] + a.wterm[kb];
             }
         });

@@ -119,7 +119,7 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
     StepArgs<T> a;
     const long long is = c->soa ? 1 : c->Q;  // elements per cell step
     for (int k = 0; k < 27; ++k) {
-        a.plane[k] = a.ldo[k] = a.sto[k] = 0;
+        a.plane[k] = a.ldo[k] = a.sto[k] = a.wlo[k] = a.wso[k] = 0;
         if (k >= c->Q) continue;
         const int kb = c->opp[k];
         const long long off = ((long long)c->c[k][0] * c->ny + c->c[k][1]) * c->nz + c->c[k][2];
@@ -128,6 +128,8 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
         a.plane[k] = pk;
         a.ldo[k] = (long long)sizeof(T) * (load == LD_LOCAL ? pk : load == LD_PULL ? pk - off * is : pkb - off * is);
         a.sto[k] = (long long)sizeof(T) * (store == ST_LOCAL ? pk : store == ST_SWAPPED ? pkb : pk + off * is);
+        a.wlo[k] = (long long)sizeof(T) * (load == LD_PULL ? pkb : pk);
+        a.wso[k] = (long long)sizeof(T) * pkb;
     }
     a.src = (const T*)src;
     a.dst = (T*)dst;
