@@ -167,8 +167,11 @@ cudaError_t aux_insert_plane(int Q, bool soa, T* pop, const uint8_t* code, const
 template <class T>
 cudaError_t aux_swap_stream(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s)
 {
-    const int grid = blocks_for(a.g.n, 256);
-#define CALL(QQ, SS) swap_stream_kernel<T, QQ, SS><<<grid, 256, 0, s>>>(a)
+#define CALL(QQ, SS)                                                                   \
+    {                                                                                  \
+        constexpr int b = swap_max_threads<T, QQ>() < 256 ? swap_max_threads<T, QQ>() : 256; \
+        swap_stream_kernel<T, QQ, SS><<<blocks_for(a.g.n, b), b, 0, s>>>(a);           \
+    }
     LBM_QS_DISPATCH(Q, soa, CALL);
 #undef CALL
     return cudaGetLastError();

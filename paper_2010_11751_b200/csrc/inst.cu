@@ -19,7 +19,8 @@ static cudaError_t launch_one(int block, bool staged, const StepArgs<T>& a, cuda
             return cudaGetLastError();
         }
     }
-    step_kernel<T, Q, MODEL, SOA, LOAD, STORE><<<(a.g.n + block - 1) / block, block, 0, s>>>(a);
+    const int b = block > max_threads<T, Q>() ? max_threads<T, Q>() : block;
+    step_kernel<T, Q, MODEL, SOA, LOAD, STORE><<<(a.g.n + b - 1) / b, b, 0, s>>>(a);
     return cudaGetLastError();
 }
 

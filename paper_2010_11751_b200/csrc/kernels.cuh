@@ -206,12 +206,18 @@ __device__ __forceinline__ CellState cell_state(const uint8_t* __restrict__ code
 }
 
 // ------------------------------------------------------------------ the fused step
-// minimum resident blocks of 256 threads per SM (register cap 65536 / (256 * n)): tuned on B200
+// __launch_bounds__(max_threads, min_blocks) = the register cap 65536 / (max_threads * min_blocks),
+// tuned on B200 per precision and lattice: fp64 D3Q19 128 x 7 (72 registers, 28 warps per SM), fp64
+// D3Q27 128 x 5 (96 registers: 20 warps per SM instead of the 16 that 128 registers allow), fp32 D3Q19 256 x 6 (40), fp32
+// D3Q27 256 x 4 (64).  Launches clamp the block size to max_threads.
 #ifndef LBM_MINB_D19
-#define LBM_MINB_D19 3
+#define LBM_MINB_D19 7
+#endif
+#ifndef LBM_MAXT_D27
+#define LBM_MAXT_D27 128
 #endif
 #ifndef LBM_MINB_D27
-#define LBM_MINB_D27 2
+#define LBM_MINB_D27 5
 #endif
 #ifndef LBM_MINB_F
 #define LBM_MINB_F 6
@@ -221,9 +227,20 @@ __device__ __forceinline__ CellState cell_state(const uint8_t* __restrict__ code
 #endif
 template <class T, int Q>
 constexpr int min_blocks() { return sizeof(T) == 4 ? (Q == 19 ? LBM_MINB_F : LBM_MINB_F27) : Q == 19 ? LBM_MINB_D19 : LBM_MINB_D27; }
+#ifndef LBM_MAXT_D19
+#define LBM_MAXT_D19 128
+#endif
+#ifndef LBM_MAXT_F
+#define LBM_MAXT_F 256
+#endif
+#ifndef LBM_MAXT_F27
+#define LBM_MAXT_F27 256
+#endif
+template <class T, int Q>
+constexpr int max_threads() { return sizeof(T) == 4 ? (Q == 19 ? LBM_MAXT_F : LBM_MAXT_F27) : Q == 19 ? LBM_MAXT_D19 : LBM_MAXT_D27; }
 
 template <class T, int Q, int MODEL, bool SOA, int LOAD, int STORE>
-__global__ void __launch_bounds__(256, min_blocks<T, Q>()) step_kernel(const StepArgs<T> a)
+__global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_kernel(const StepArgs<T> a)
 {
     constexpr bool SHIFT = sizeof(T) == 4;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -297,11 +314,20 @@ __global__ void __launch_bounds__(128) step_kernel_aos(const StepArgs<T> a)
 // Every slot is touched by exactly one thread (Table 1), so all loads
 // are issued before the first store.
 // resident blocks of 256 threads per SM for pass 2 (register cap), tuned on B200: fp64 3 / 2 (D3Q19 / D3Q27),
-// fp32 4 / 3.  Uncapped, the D3Q27 fp64 instance took 144 registers (one block per SM, 65 % of the copy rate).
+// fp32 4 / 3; the D3Q27 fp64 instance 128 x 5 (96 registers).  Uncapped it took 144 registers (one block of 256
+// per SM, 65 % of the copy rate).
+#ifndef LBM_SWAP_MAXT_D27
+#define LBM_SWAP_MAXT_D27 128
+#endif
+#ifndef LBM_SWAP_MINB_D27
+#define LBM_SWAP_MINB_D27 5
+#endif
 template <class T, int Q>
-constexpr int swap_min_blocks() { return (sizeof(T) == 8 ? 3 : 4) - (Q == 27 ? 1 : 0); }
+constexpr int swap_max_threads() { return (sizeof(T) == 8 && Q == 27) ? LBM_SWAP_MAXT_D27 : 256; }
+template <class T, int Q>
+constexpr int swap_min_blocks() { return (sizeof(T) == 8 && Q == 27) ? LBM_SWAP_MINB_D27 : (sizeof(T) == 8 ? 3 : 4) - (Q == 27 ? 1 : 0); }
 template <class T, int Q, bool SOA>
-__global__ void __launch_bounds__(256, swap_min_blocks<T, Q>()) swap_stream_kernel(const StepArgs<T> a)
+__global__ void __launch_bounds__(swap_max_threads<T, Q>(), swap_min_blocks<T, Q>()) swap_stream_kernel(const StepArgs<T> a)
 {
     using L = Lat<Q>;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -398,7 +424,7 @@ __global__ void macroscopic_kernel(const T* __restrict__ pop, const uint8_t* __r
 // kinetic energy, stage 1: one cell per thread, one double per block of 256 cells (fixed tree: warp
 // shuffle, then warp 0), so that as many loads are in flight as in the step kernels
 template <class T, int Q, bool SOA, int LOAD>
-__global__ void __launch_bounds__(256, min_blocks<T, Q>()) energy_kernel(const T* __restrict__ pop, const uint8_t* __restrict__ code, Geo g,
+__global__ void __launch_bounds__(256) energy_kernel(const T* __restrict__ pop, const uint8_t* __restrict__ code, Geo g,
                                                                          StepArgs<T> a, double* __restrict__ partial)
 {
     constexpr bool SHIFT = sizeof(T) == 4;
