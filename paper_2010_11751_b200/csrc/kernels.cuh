@@ -424,7 +424,7 @@ __global__ void macroscopic_kernel(const T* __restrict__ pop, const uint8_t* __r
 // kinetic energy, stage 1: one cell per thread, one double per block of 256 cells (fixed tree: warp
 // shuffle, then warp 0), so that as many loads are in flight as in the step kernels
 template <class T, int Q, bool SOA, int LOAD>
-__global__ void __launch_bounds__(256) energy_kernel(const T* __restrict__ pop, const uint8_t* __restrict__ code, Geo g,
+__global__ void __launch_bounds__(256, sizeof(T) == 8 ? (Q == 19 ? 3 : 2) : (Q == 19 ? 6 : 4)) energy_kernel(const T* __restrict__ pop, const uint8_t* __restrict__ code, Geo g,
                                                                          StepArgs<T> a, double* __restrict__ partial)
 {
     constexpr bool SHIFT = sizeof(T) == 4;
