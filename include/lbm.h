@@ -57,7 +57,7 @@ int lbm_set_hooks(lbm_alloc_fn alloc, lbm_free_fn free_fn, void* stream);
  * model, a scheme, the shear relaxation rate omega in (0,2) with nu = (1/omega - 1/2)/3
  * and the storage/arithmetic type.  All cells start FLUID (fully periodic box).
  * Default rates (R14): omega_bulk = omega, moments of order >= 3 relaxed with 1 (RR: with omega);
- * TRT magic parameter 1/4 (R15).  LBM_F32 is available for BGK_W2, TRT and REG. */
+ * TRT magic parameter 1/4 (R15).  LBM_F32 stores and computes on f_k - t_k (R20). */
 lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme, double omega, int dtype);
 int lbm_destroy(lbm_t* ctx);
 

@@ -1,6 +1,6 @@
 // inst.cu -- step kernels of ONE (lattice, collision model) pair; compiled once per pair with
 //   -DLBM_INST_Q=<19|27> -DLBM_INST_MODEL=<0..9>
-// (see paper_2010_11751_b200/build.py).  fp64 always; fp32 for the W2 family (BGK_W2, TRT, REG).
+// (see paper_2010_11751_b200/build.py).  fp64 and fp32 (shifted storage, R20).
 #include "dispatch.cuh"
 
 #ifndef LBM_INST_Q
@@ -45,8 +45,6 @@ cudaError_t launch_step(int kind, bool soa, int block, bool staged, const StepAr
 }
 
 template cudaError_t launch_step<double, LBM_INST_Q, LBM_INST_MODEL>(int, bool, int, bool, const StepArgs<double>&, cudaStream_t);
-#if LBM_INST_MODEL == 0 || LBM_INST_MODEL == 2 || LBM_INST_MODEL == 9
 template cudaError_t launch_step<float, LBM_INST_Q, LBM_INST_MODEL>(int, bool, int, bool, const StepArgs<float>&, cudaStream_t);
-#endif
 
 }  // namespace lbm

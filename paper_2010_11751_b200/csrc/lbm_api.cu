@@ -163,7 +163,7 @@ cudaError_t step_model(const lbm_ctx* c, int kind, const StepArgs<T>& a)
     case LBM_REG: return launch_step<T, Q, M_REG>(kind, soa, b, st, a, s);
     default: break;
     }
-    if constexpr (sizeof(T) == 8) {
+    {
         switch (c->model) {
         case LBM_BGK_NW4: return launch_step<T, Q, M_BGK_NW4>(kind, soa, b, st, a, s);
         case LBM_RM: return launch_step<T, Q, M_RM>(kind, soa, b, st, a, s);
@@ -345,10 +345,6 @@ lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme
     if (scheme < 0 || scheme >= LBM_NUM_SCHEMES) { set_err("unknown scheme %d", scheme); return nullptr; }
     if (dtype != LBM_F32 && dtype != LBM_F64) { set_err("dtype must be LBM_F32 or LBM_F64"); return nullptr; }
     if (!(omega > 0.0 && omega < 2.0)) { set_err("omega must be in (0,2)"); return nullptr; }
-    if (dtype == LBM_F32 && !model_is_w2(collision)) {
-        set_err("fp32 is available for BGK_W2, TRT and REG only");
-        return nullptr;
-    }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
         set_err("no CUDA device: this library has no CPU fallback");

@@ -65,6 +65,8 @@ def groups():
                    for b in (64, 128, 256)]
     g["misc27"] = [case(192, Q=27, model=m, scheme=s, dtype="f32") for m in ("BGK_W2", "TRT", "REG")
                    for s in ("2POP_SOA", "AA_SOA", "SWAP_SOA")] + [case(192, Q=27, scheme="2POP_SOA")]
+    g["models_f32"] = [case(256, model=m, scheme="AA_SOA", dtype="f32") for m in ALL_MODELS] + \
+                      [case(192, Q=27, model=m, scheme="AA_SOA", dtype="f32") for m in ALL_MODELS]
     g["small"] = [case(n, scheme=s, omega=inputs.omega_from_re(32, 100)) for s in ("2POP_SOA", "AA_SOA", "SWAP_SOA")
                   for n in (16, 32, 48, 64)]
     return g

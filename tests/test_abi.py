@@ -69,7 +69,9 @@ def test_create_rejects_bad_arguments_without_gpu(lib_path):
     assert lib.lbm_create(8, 8, 8, 19, 10, 0, 1.0, 1) is None
     assert lib.lbm_create(8, 8, 8, 19, 0, 6, 1.0, 1) is None
     assert lib.lbm_create(8, 8, 8, 19, 0, 0, 2.5, 1) is None and b"omega" in lib.lbm_last_error()
-    assert lib.lbm_create(8, 8, 8, 19, 7, 0, 1.0, 0) is None and b"fp32" in lib.lbm_last_error()
+    assert lib.lbm_create(8, 8, 8, 19, 7, 0, 1.0, 2) is None and b"dtype" in lib.lbm_last_error()
+    # a valid request still fails loudly here: no device, no CPU fallback
+    assert lib.lbm_create(8, 8, 8, 19, 7, 0, 1.0, 0) is None and b"no CPU fallback" in lib.lbm_last_error()
 
 
 def test_product_never_imports_oracle():
