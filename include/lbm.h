@@ -139,11 +139,12 @@ long long lbm_halo_count(const lbm_t* ctx);
 int lbm_halo_pack(lbm_t* ctx, int face, void* buf_dev);
 int lbm_halo_unpack(lbm_t* ctx, int face, const void* buf_dev);
 
-/* CUDA-graph replay of lbm_step.  A step of a lattice below ~96^3 cells lasts a few microseconds
- * and is bound by launch latency (the paper's "one synchronisation per step");
- * lbm_step(n) then captures 16 steps once and replays the graph.  LBM_GRAPH_AUTO (default): only
- * for such small lattices; LBM_GRAPH_OFF: never; LBM_GRAPH_ON: for any size.  Results are
- * identical (same kernels, same order).  lbm_graph_replays = graph launches so far. */
+/* CUDA-graph replay of lbm_step.  A step of a small lattice lasts a few microseconds and is bound
+ * by launch latency (the paper's "one synchronisation per step"), and up to ~128^3
+ * the gaps between launches still cost 2-5 %; lbm_step(n) then captures 16 steps once and replays
+ * the graph.  LBM_GRAPH_AUTO (default): lattices of at most 160^3 cells; LBM_GRAPH_OFF: never;
+ * LBM_GRAPH_ON: any size.  Results are identical (same kernels, same order).  lbm_graph_replays =
+ * graph launches so far. */
 enum { LBM_GRAPH_AUTO = 0, LBM_GRAPH_OFF = 1, LBM_GRAPH_ON = 2 };
 int lbm_set_graph(lbm_t* ctx, int mode);
 long long lbm_graph_replays(const lbm_t* ctx);

@@ -255,7 +255,7 @@ int one_step(lbm_ctx* c)
 // baked in) and replayed; every scheme returns to the same storage state and the same pop[0]
 // after an even number of steps, so one graph serves the whole run.  Any call that changes what
 // the kernels would be given (rates, flags, variant, block, populations' home) drops the graph.
-enum { GRAPH_STEPS = 16, GRAPH_AUTO_MAX_CELLS = 96 * 96 * 96 };
+enum { GRAPH_STEPS = 16, GRAPH_AUTO_MAX_CELLS = 160 * 160 * 160 };
 
 void drop_graph(lbm_ctx* c)
 {
