@@ -25,7 +25,7 @@
  * magic parameter 1/4, W2 equilibrium), R16 (Eq 12 is rho*M), R17 (D3Q27 as the tensor
  * product extension), R18 (REG), R19 (kinetic energy = sum_fluid 1/2 rho |u|^2).
  *
- * Pins (tests/test_oracle_*.py): P1..P15 of SURVEY.md 8(c).  Parity with the authors'
+ * Pins (tests/test_oracle_*.py): P1..P15 of SURVEY.md 8(c), P16..P18 of DESIGN.md 5.  Parity with the authors'
  * own code for RM/HM/CM/CHM/K/RR/NW4 beyond those pins is "parity unpinned": Ref [31]
  * App. G and the stlbm sources are not available.
  *

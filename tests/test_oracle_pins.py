@@ -310,6 +310,58 @@ def test_p15_rr_equals_chm_and_hm_limits(oracle, Q):
 
 
 @pytest.mark.parametrize("Q", LATTICES)
+@pytest.mark.parametrize("model", ["BGK_NW4", "RM", "HM", "CM", "CHM", "K", "RR"])
+def test_p16_all_rates_one_returns_the_extended_equilibrium(oracle, Q, model):
+    """every moment-space model with every rate equal to 1 projects any population onto the extended
+    equilibrium of its own rho and u ("omega = 1 ... equilibrates"): independent of the
+    basis and, for the cumulants, of the non-linear moment <-> cumulant maps"""
+    rng = np.random.default_rng(21)
+    c, *_ = oracle.lattice(Q)
+    f = perturbed(oracle, Q, model, rng, amp=5e-2)
+    rho = f.sum()
+    u = (c.T @ f) / rho
+    out = oracle.collide(Q, model, f, 1.0, omega_bulk=1.0, omega3=1.0, omega_hi=1.0)
+    assert np.abs(out - oracle.equilibrium(Q, "ext", rho, u)).max() < 2e-15
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+@pytest.mark.parametrize("model", ALL_MODELS)
+def test_p17_second_order_nonequilibrium_stress_scales_by_one_minus_omega(oracle, Q, model):
+    """nu = (1/omega - 1/2) c_s^2 for EVERY model: with omega_bulk = omega the
+    non-equilibrium second moment Pi = sum c c f - rho (u u + c_s^2 I), computed here from plain
+    sums over the populations, leaves the collision multiplied by (1 - omega), whatever the basis"""
+    rng = np.random.default_rng(22)
+    c, *_ = oracle.lattice(Q)
+    f = perturbed(oracle, Q, model, rng, amp=3e-2)
+
+    def pi_neq(g):
+        rho = g.sum()
+        u = (c.T @ g) / rho
+        return np.einsum("ka,kb,k->ab", c, c, g) - rho * (np.outer(u, u) + np.eye(3) / 3.0)
+
+    for omega in (0.7, 1.6, 1.95):
+        out = oracle.collide(Q, model, f, omega)
+        assert np.abs(pi_neq(out) - (1.0 - omega) * pi_neq(f)).max() < 1e-15
+
+
+@pytest.mark.parametrize("Q", LATTICES)
+def test_p18_cumulants_differ_from_central_moments_from_fourth_order_on(oracle, Q):
+    """cumulants and central moments coincide up to third order, so K and CM at the same rates must
+    leave identical central moments of order <= 3 and may differ only above"""
+    rng = np.random.default_rng(23)
+    c, t, opp, mom = oracle.lattice(Q)
+    f = perturbed(oracle, Q, "K", rng, amp=5e-2)
+    kw = dict(omega_bulk=1.2, omega3=1.4, omega_hi=0.9)
+    a = oracle.collide(Q, "K", f, 1.7, **kw)
+    b = oracle.collide(Q, "CM", f, 1.7, **kw)
+    u = (c.T @ f) / f.sum()
+    ka, kb = oracle.moments(Q, "central", a, u), oracle.moments(Q, "central", b, u)
+    order = np.array([sum(m) for m in mom])
+    assert np.abs(ka - kb)[order <= 3].max() < 1e-15
+    assert np.abs(ka - kb)[order >= 4].max() > 1e-9
+
+
+@pytest.mark.parametrize("Q", LATTICES)
 def test_bulk_rate_eq13_15(oracle, Q):
     """Eq 13-15: trace of the second-order non-equilibrium relaxes with omega_bulk, the deviator with omega;
     with omega_bulk = omega the three equations reduce to Eq 11 (R3)."""
