@@ -135,6 +135,16 @@ int lbm_set_block(lbm_t* ctx, int threads);
  * buf is DEVICE memory of lbm_halo_count() elements of the context dtype, layout [dir][ny*nz] with
  * directions in increasing k; asynchronous on the stream.  Two-population SoA scheme only
  * (LBM_E_ARG otherwise); raw stored values, so both ranks must use the same dtype. */
+/* One time step in two parts, so that the halo exchange overlaps the bulk of the update:
+ *   lbm_step_begin   updates the outermost owned layers x = 1 and x = nx-2 only;
+ *   lbm_halo_pack    (both faces) then reads the new values of those layers; start the exchange;
+ *   lbm_step_end     updates the layers 2 .. nx-3 and completes the step;
+ *   lbm_halo_unpack  (both faces) once the neighbours' buffers have arrived.
+ * Layers 0 and nx-1 are not updated by this pair: they must be GHOST or solid.  The result is
+ * bit for bit that of lbm_step(1).  Between begin and end only lbm_halo_pack is allowed
+ * (LBM_E_STATE otherwise).  Two-population SoA scheme only. */
+int lbm_step_begin(lbm_t* ctx);
+int lbm_step_end(lbm_t* ctx);
 long long lbm_halo_count(const lbm_t* ctx);
 int lbm_halo_pack(lbm_t* ctx, int face, void* buf_dev);
 int lbm_halo_unpack(lbm_t* ctx, int face, const void* buf_dev);

@@ -27,7 +27,7 @@ SYMBOLS = [
     "lbm_set_hooks", "lbm_create", "lbm_destroy", "lbm_set_flags", "lbm_set_relaxation", "lbm_set_trt_magic",
     "lbm_init_equilibrium", "lbm_init_equilibrium_device", "lbm_step", "lbm_macroscopic", "lbm_macroscopic_device", "lbm_kinetic_energy", "lbm_get_populations", "lbm_get_populations_at",
     "lbm_set_populations", "lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches",
-    "lbm_sync", "lbm_set_variant", "lbm_set_block", "lbm_set_graph", "lbm_graph_replays", "lbm_halo_count", "lbm_halo_pack", "lbm_halo_unpack", "lbm_last_error", "lbm_version",
+    "lbm_sync", "lbm_set_variant", "lbm_set_block", "lbm_set_graph", "lbm_graph_replays", "lbm_halo_count", "lbm_halo_pack", "lbm_halo_unpack", "lbm_step_begin", "lbm_step_end", "lbm_last_error", "lbm_version",
 ]
 GRAPH_MODES = {"auto": 0, "off": 1, "on": 2}
 
@@ -70,6 +70,8 @@ def load_library(path=LIB_PATH):
     L.lbm_get_populations_at.argtypes = [vp, vp, i, vp]
     L.lbm_set_populations.argtypes = [vp, vp]
     L.lbm_set_graph.argtypes = [vp, i]
+    L.lbm_step_begin.argtypes = [vp]
+    L.lbm_step_end.argtypes = [vp]
     L.lbm_halo_count.restype = C.c_longlong
     L.lbm_halo_count.argtypes = [vp]
     L.lbm_halo_pack.argtypes = [vp, i, vp]
@@ -235,6 +237,13 @@ class Lbm:
     @property
     def kernel_launches(self):
         return self._L.lbm_kernel_launches(self._h)
+
+    def step_begin(self):
+        """outermost owned x-layers of the next step (slab overlap; see include/lbm.h)"""
+        self._ck(self._L.lbm_step_begin(self._h))
+
+    def step_end(self):
+        self._ck(self._L.lbm_step_end(self._h))
 
     @property
     def halo_count(self):

@@ -13,14 +13,14 @@ template <class T, int Q, int MODEL, bool SOA, int LOAD, int STORE>
 static cudaError_t launch_one(int block, bool staged, const StepArgs<T>& a, cudaStream_t s)
 {
     if constexpr (!SOA && (LOAD == LD_LOCAL || STORE != ST_PUSH)) {
-        if (staged) {  // AoS: local accesses through a transposing shared-memory tile (kernels.cuh)
+        if (staged && a.first == 0 && a.end == a.g.n) {  // AoS: local accesses through a transposing shared-memory tile (kernels.cuh)
             const int b = block > 128 ? 128 : block;
             step_kernel_aos<T, Q, MODEL, LOAD, STORE><<<(a.g.n + b - 1) / b, b, (size_t)b * Q * sizeof(T), s>>>(a);
             return cudaGetLastError();
         }
     }
     const int b = block > max_threads<T, Q>() ? max_threads<T, Q>() : block;
-    step_kernel<T, Q, MODEL, SOA, LOAD, STORE><<<(a.g.n + b - 1) / b, b, 0, s>>>(a);
+    step_kernel<T, Q, MODEL, SOA, LOAD, STORE><<<(a.end - a.first + b - 1) / b, b, 0, s>>>(a);
     return cudaGetLastError();
 }
 

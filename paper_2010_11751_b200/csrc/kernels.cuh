@@ -47,6 +47,7 @@ struct StepArgs {
     const uint8_t* code;
     const unsigned long long* mask;
     Geo g;
+    int first, end;   // the step kernel updates the cells [first, end): the whole box, or some x-layers (slab overlap)
     Rates<T> rt;
     T wterm[27];  // w_k
     // offsets filled on the host per launch (make_args) so that the kernels add one uniform
@@ -243,8 +244,8 @@ template <class T, int Q, int MODEL, bool SOA, int LOAD, int STORE>
 __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_kernel(const StepArgs<T> a)
 {
     constexpr bool SHIFT = sizeof(T) == 4;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
+    const int i = a.first + blockIdx.x * blockDim.x + threadIdx.x;
+    const CellState cs = cell_state(a.code, a.mask, i, a.end);
     if (!cs.active) {  // solid cells hold no populations
         // ... but when the other array is written (two-population), a warp that straddles a wall
         // fills the wall cells' slots too: a partially written 32 B sector that is not in L2 costs

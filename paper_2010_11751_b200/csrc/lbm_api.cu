@@ -66,6 +66,8 @@ struct lbm_ctx {
     // CUDA-graph replay of lbm_step for launch-bound lattices (see step_graphed)
     int graph_mode;             // LBM_GRAPH_AUTO / OFF / ON
     cudaGraphExec_t graph_exec; // GRAPH_STEPS steps starting from graph_sto with pop[0] == graph_pop0
+    int range_first, range_end;  // cells the next step launch covers (0, 0 = all); lbm_step_begin / lbm_step_end
+    bool mid_step;               // between lbm_step_begin and lbm_step_end
     cudaStream_t cap_stream;    // private stream the capture runs on (the context stream may be the
                                 // legacy default stream, which cannot be captured); nothing executes on it
     Storage graph_sto;
@@ -136,6 +138,8 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
     a.code = c->code;
     a.mask = c->mask;
     a.g = c->g;
+    a.first = c->range_first;
+    a.end = c->range_end > 0 ? c->range_end : c->g.n;
     a.rt.omega = (T)c->omega;
     a.rt.omega_bulk = (T)c->omega_bulk;
     a.rt.omega3 = (T)c->omega3;
@@ -472,6 +476,7 @@ int lbm_init_equilibrium_device(lbm_t* c, const void* rho, const void* u)
     c->launches++;
     c->sto = STO_CANON;
     c->steps = 0;
+    c->mid_step = false;
     return LBM_OK;
 }
 
@@ -492,6 +497,7 @@ int lbm_step(lbm_t* c, int n)
     if (!c) { set_err("null context"); return LBM_E_ARG; }
     if (n < 0) { set_err("n must be >= 0"); return LBM_E_ARG; }
     if (c->sto == STO_NONE) { set_err("lbm_step before lbm_init_equilibrium / lbm_set_populations"); return LBM_E_STATE; }
+    if (c->mid_step) { set_err("lbm_step between lbm_step_begin and lbm_step_end"); return LBM_E_STATE; }
     int s = 0;
     if (graph_wanted(c, n)) {
         // the graph covers an even number of steps from a periodic state: get there first
@@ -523,6 +529,7 @@ long long lbm_graph_replays(const lbm_t* c) { return c ? c->graph_replays : -1; 
 int lbm_macroscopic_device(lbm_t* c, void* rho, void* u)
 {
     if (!c || !rho || !u) { set_err("null argument"); return LBM_E_ARG; }
+    if (c->mid_step) { set_err("export between lbm_step_begin and lbm_step_end"); return LBM_E_STATE; }
     if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
     if (c->dtype == LBM_F64)
         CK(aux_macroscopic<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr, load_mode(c)), (double*)rho,
@@ -549,6 +556,7 @@ int lbm_macroscopic(lbm_t* c, void* rho, void* u)
 int lbm_kinetic_energy(lbm_t* c, double* e)
 {
     if (!c || !e) { set_err("null argument"); return LBM_E_ARG; }
+    if (c->mid_step) { set_err("export between lbm_step_begin and lbm_step_end"); return LBM_E_STATE; }
     if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
     if (c->dtype == LBM_F64)
         CK(aux_energy<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr, load_mode(c)), c->partial,
@@ -565,6 +573,7 @@ int lbm_kinetic_energy(lbm_t* c, double* e)
 // canonical planes f_k of the whole box (cells_dev == nullptr, m = N) or of m listed cells
 static int export_planes(lbm_t* c, void* f, const int* cells_dev, int m)
 {
+    if (c->mid_step) { set_err("export between lbm_step_begin and lbm_step_end"); return LBM_E_STATE; }
     const size_t nb = (size_t)m * c->elem;
     const size_t plane = (size_t)c->g.n * c->elem;
     const int mode = load_mode(c);
@@ -660,6 +669,46 @@ static HaloArgs halo_args(const lbm_t* c, int want_cx, int x_layer)
     p.first = (long long)x_layer * p.cells;
     return p;
 }
+// one launch of the two-population pull step over the x-layers [xa, xb), nothing committed
+static int step_layers(lbm_t* c, int xa, int xb)
+{
+    if (xb <= xa) return LBM_OK;
+    const int layer = c->ny * c->nz;
+    c->range_first = xa * layer;
+    c->range_end = xb * layer;
+    cudaError_t e = c->sto == STO_CANON ? step_kind(c, SK_COLLIDE, c->pop[0], c->pop[0])
+                                        : step_kind(c, SK_PULL, c->pop[0], c->pop[1]);
+    c->range_first = c->range_end = 0;
+    if (e != cudaSuccess) return cuda_fail("step_layers", e);
+    return LBM_OK;
+}
+int lbm_step_begin(lbm_t* c)
+{
+    if (!c) { set_err("null context"); return LBM_E_ARG; }
+    if (c->scheme != LBM_2POP_SOA || !use_pull(c)) {
+        set_err("lbm_step_begin / lbm_step_end are implemented for the two-population SoA scheme (pull form) only");
+        return LBM_E_ARG;
+    }
+    if (c->sto == STO_NONE) { set_err("lbm_step_begin before lbm_init_equilibrium / lbm_set_populations"); return LBM_E_STATE; }
+    if (c->mid_step) { set_err("lbm_step_begin twice"); return LBM_E_STATE; }
+    if (int rc = step_layers(c, 1, 2)) return rc;
+    if (c->nx - 2 > 1)
+        if (int rc = step_layers(c, c->nx - 2, c->nx - 1)) return rc;
+    c->mid_step = true;
+    return LBM_OK;
+}
+int lbm_step_end(lbm_t* c)
+{
+    if (!c) { set_err("null context"); return LBM_E_ARG; }
+    if (!c->mid_step) { set_err("lbm_step_end without lbm_step_begin"); return LBM_E_STATE; }
+    if (int rc = step_layers(c, 2, c->nx - 2)) return rc;
+    if (c->sto == STO_CANON) c->sto = STO_POST;
+    else { void* t = c->pop[0]; c->pop[0] = c->pop[1]; c->pop[1] = t; }
+    c->mid_step = false;
+    c->steps++;
+    return LBM_OK;
+}
+
 long long lbm_halo_count(const lbm_t* c)
 {
     if (!c) return -1;
@@ -670,14 +719,17 @@ int lbm_halo_pack(lbm_t* c, int face, void* buf)
     if (int rc = halo_check(c, face, buf)) return rc;
     // populations that leave through the face: cx = -1 from the first owned layer (x = 1), cx = +1 from the last (x = nx-2)
     const HaloArgs p = halo_args(c, face == 0 ? -1 : +1, face == 0 ? 1 : c->nx - 2);
-    if (c->dtype == LBM_F64) CK(aux_halo<double>(true, (double*)c->pop[0], c->g.stride, p, (double*)buf, c->stream));
-    else CK(aux_halo<float>(true, (float*)c->pop[0], c->g.stride, p, (float*)buf, c->stream));
+    // between lbm_step_begin and lbm_step_end the new values of the outer layers sit in the array being written
+    void* from = (c->mid_step && c->sto == STO_POST) ? c->pop[1] : c->pop[0];
+    if (c->dtype == LBM_F64) CK(aux_halo<double>(true, (double*)from, c->g.stride, p, (double*)buf, c->stream));
+    else CK(aux_halo<float>(true, (float*)from, c->g.stride, p, (float*)buf, c->stream));
     c->launches++;
     return LBM_OK;
 }
 int lbm_halo_unpack(lbm_t* c, int face, const void* buf)
 {
     if (int rc = halo_check(c, face, buf)) return rc;
+    if (c->mid_step) { set_err("lbm_halo_unpack between lbm_step_begin and lbm_step_end"); return LBM_E_STATE; }
     // populations that enter through the face: cx = +1 into the low ghost layer (x = 0), cx = -1 into the high one (x = nx-1)
     const HaloArgs p = halo_args(c, face == 0 ? +1 : -1, face == 0 ? 0 : c->nx - 1);
     if (c->dtype == LBM_F64) CK(aux_halo<double>(false, (double*)c->pop[0], c->g.stride, p, (double*)buf, c->stream));

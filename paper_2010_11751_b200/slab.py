@@ -92,25 +92,57 @@ def exchange_local(engines):
         e.halo_unpack(1, sent[right][0])   # what left the right neighbour through its low face
 
 
-def exchange_dist(engine, dist, rank, world, group=None):
-    """the same over torch.distributed, one slab per process.  Buffers are torch tensors on the
-    backend's device (CUDA for nccl, CPU for gloo); the engine offers halo_pack(face) -> tensor,
-    halo_recv_buffer(face) -> tensor and halo_unpack(face, tensor)."""
+def exchange_start(engine, dist, rank, world, group=None):
+    """pack both faces and post the sends / receives; returns a handle for exchange_finish.  Over
+    nccl the transfers run on the communicator's own stream, so whatever the caller launches next
+    on the compute stream (lbm_step_end: the interior of the slab) overlaps them."""
     s0, s1 = engine.halo_pack(0), engine.halo_pack(1)
     r0, r1 = engine.halo_recv_buffer(0), engine.halo_recv_buffer(1)
     if world == 1:
         r0.copy_(s1)
         r1.copy_(s0)
-    else:
-        left, right = neighbours(rank, world)
-        # the message tag is the face it LEFT through; nccl ignores tags and matches in order, so
-        # with two ranks (left == right) the receives are posted in the peer's send order
-        ops = [dist.P2POp(dist.isend, s0, left, group, 0), dist.P2POp(dist.isend, s1, right, group, 1),
-               dist.P2POp(dist.irecv, r1, right, group, 0), dist.P2POp(dist.irecv, r0, left, group, 1)]
-        for req in dist.batch_isend_irecv(ops):
-            req.wait()
+        return (r0, r1, [])
+    left, right = neighbours(rank, world)
+    # the message tag is the face it LEFT through; nccl ignores tags and matches in order, so
+    # with two ranks (left == right) the receives are posted in the peer's send order
+    ops = [dist.P2POp(dist.isend, s0, left, group, 0), dist.P2POp(dist.isend, s1, right, group, 1),
+           dist.P2POp(dist.irecv, r1, right, group, 0), dist.P2POp(dist.irecv, r0, left, group, 1)]
+    return (r0, r1, dist.batch_isend_irecv(ops))
+
+
+def exchange_finish(engine, handle):
+    r0, r1, reqs = handle
+    for req in reqs:
+        req.wait()
     engine.halo_unpack(0, r0)
     engine.halo_unpack(1, r1)
+
+
+def exchange_dist(engine, dist, rank, world, group=None):
+    """the exchange over torch.distributed, one slab per process.  Buffers are torch tensors on the
+    backend's device (CUDA for nccl, CPU for gloo); the engine offers halo_pack(face) -> tensor,
+    halo_recv_buffer(face) -> tensor and halo_unpack(face, tensor)."""
+    exchange_finish(engine, exchange_start(engine, dist, rank, world, group))
+
+
+def step_local(engines, overlap=True):
+    """one time step of several GPU slabs living in this process.  overlap = the order a multi-GPU
+    run uses: outer layers, pack, interior, unpack (lbm_step_begin / lbm_step_end)."""
+    W = len(engines)
+    if overlap:
+        for e in engines:
+            e.lbm.step_begin()
+        sent = [(e.halo_pack(0), e.halo_pack(1)) for e in engines]
+        for e in engines:
+            e.lbm.step_end()
+        for r, e in enumerate(engines):
+            left, right = neighbours(r, W)
+            e.halo_unpack(0, sent[left][1])
+            e.halo_unpack(1, sent[right][0])
+    else:
+        for e in engines:
+            e.lbm.step(1)
+        exchange_local(engines)
 
 
 class GpuSlabEngine:
@@ -151,10 +183,11 @@ class SlabLbm:
     (kinetic energy)."""
 
     def __init__(self, NX, NY, NZ, flags=None, u_wall=(0.0, 0.0, 0.0), dist=None, rank=0, world=1, group=None,
-                 lattice=19, collision="BGK_W2", omega=1.0, dtype="f64", flags_local=None):
+                 lattice=19, collision="BGK_W2", omega=1.0, dtype="f64", flags_local=None, overlap=True):
         """flags: GLOBAL [NX, NY, NZ] (None = all fluid), or flags_local: this rank's [nxl+2, NY, NZ]
         with its ghost layers already in place (local_flags / cavity_slab)"""
         self.dist, self.rank, self.world, self.group = dist, rank, world, group
+        self.overlap = overlap    # exchange the halo while the interior of the slab is updated
         self.N = (NX, NY, NZ)
         self.x0, self.x1 = slab_range(NX, rank, world)
         if flags_local is not None:
@@ -179,16 +212,17 @@ class SlabLbm:
         """rho [nxl+2, NY, NZ], u [3, nxl+2, NY, NZ] of this rank's context, ghost layers included"""
         self.lbm.init_equilibrium(np.asarray(rho_local, dtype=self.engine.np_dtype), np.asarray(u_local, dtype=self.engine.np_dtype))
 
-    def exchange(self):
-        if self.dist is None or self.world == 1:
-            exchange_local([self.engine])
-        else:
-            exchange_dist(self.engine, self.dist, self.rank, self.world, self.group)
-
     def step(self, n=1):
+        world = self.world if self.dist is not None else 1
         for _ in range(n):
-            self.lbm.step(1)
-            self.exchange()
+            if self.overlap:
+                self.lbm.step_begin()                       # the two outermost owned layers
+                h = exchange_start(self.engine, self.dist, self.rank, world, self.group)
+                self.lbm.step_end()                         # the interior, while the halo travels
+                exchange_finish(self.engine, h)
+            else:
+                self.lbm.step(1)
+                exchange_dist(self.engine, self.dist, self.rank, world, self.group)
 
     def macroscopic(self):
         """(rho [nxl, NY, NZ], u [3, nxl, NY, NZ]) of the owned layers"""

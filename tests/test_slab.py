@@ -137,8 +137,8 @@ def _flags(kind, NX, NY, NZ):
 @pytest.mark.gpu
 @pytest.mark.parametrize("Q,dtype", [(19, "f64"), (27, "f64"), (19, "f32")])
 @pytest.mark.parametrize("kind", ["cavity", "obstacle"])
-@pytest.mark.parametrize("world", [1, 2, 3])
-def test_slabs_match_the_undivided_oracle(oracle, Q, dtype, kind, world):
+@pytest.mark.parametrize("world,overlap", [(1, True), (2, False), (2, True), (3, True)])
+def test_slabs_match_the_undivided_oracle(oracle, Q, dtype, kind, world, overlap):
     NX, NY, NZ, omega, steps = 10, 9, 8, 1.7, 9
     fl, uw = _flags(kind, NX, NY, NZ)
     rho, u = inputs.seeded_init(NX, NY, NZ, 2)
@@ -158,9 +158,7 @@ def test_slabs_match_the_undivided_oracle(oracle, Q, dtype, kind, world):
         engines.append(e)
         ranges.append((x0, x1))
     for _ in range(steps):
-        for e in engines:
-            e.lbm.step(1)
-        slab.exchange_local(engines)
+        slab.step_local(engines, overlap=overlap)   # overlap: outer layers, pack, interior, unpack
     energy, nfluid = 0.0, 0
     _, t, _, _ = oracle.lattice(Q)
     for e, (x0, x1) in zip(engines, ranges):
@@ -209,6 +207,30 @@ def test_slab_lbm_single_rank_ring(oracle):
 
 
 @pytest.mark.gpu
+def test_step_begin_end_state_machine():
+    from paper_2010_11751_b200 import Lbm
+    from paper_2010_11751_b200.binding import LbmError
+    fl = slab.local_flags(inputs.cavity_flags(8, 6, 6), 2, 6)
+    g = Lbm(6, 6, 6, scheme="2POP_SOA", omega=1.5)
+    g.set_flags(fl, (0.02, 0, 0))
+    rho, u = inputs.seeded_init(6, 6, 6, 0)
+    with pytest.raises(LbmError):
+        g.step_begin()                      # nothing loaded yet
+    g.init_equilibrium(rho, u)
+    with pytest.raises(LbmError):
+        g.step_end()                        # no begin
+    g.step_begin()
+    for bad in (g.step_begin, lambda: g.step(1), g.kinetic_energy, g.macroscopic, g.get_populations):
+        with pytest.raises(LbmError):
+            bad()
+    g.step_end()
+    assert g.steps_done == 1
+    g.step(2)
+    assert g.steps_done == 3 and np.isfinite(g.kinetic_energy())
+    g.close()
+
+
+@pytest.mark.gpu
 def test_halo_api_rejects_other_schemes():
     import torch
     from paper_2010_11751_b200 import Lbm
@@ -219,6 +241,8 @@ def test_halo_api_rejects_other_schemes():
     buf = torch.empty(g.halo_count, dtype=torch.float64, device="cuda")
     with pytest.raises(LbmError):
         g.halo_pack(0, buf.data_ptr())
+    with pytest.raises(LbmError):
+        g.step_begin()
     g.close()
 
 
@@ -251,9 +275,7 @@ def test_slabs_equal_the_undivided_gpu_run_bitwise(Q, model):
         engines.append(e)
         ranges.append((x0, x1))
     for _ in range(steps):
-        for e in engines:
-            e.lbm.step(1)
-        slab.exchange_local(engines)
+        slab.step_local(engines, overlap=True)
     energy = 0.0
     for e, (x0, x1) in zip(engines, ranges):
         got = slab.interior(e.lbm.get_populations().reshape(Q, x1 - x0 + 2, NY, NZ), axis=1)
