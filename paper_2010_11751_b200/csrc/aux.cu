@@ -167,10 +167,11 @@ cudaError_t aux_insert_plane(int Q, bool soa, T* pop, const uint8_t* code, const
 template <class T>
 cudaError_t aux_swap_stream(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s)
 {
+    constexpr int G = swap_groups<T>();
 #define CALL(QQ, SS)                                                                   \
     {                                                                                  \
-        constexpr int b = swap_max_threads<T, QQ>() < 256 ? swap_max_threads<T, QQ>() : 256; \
-        swap_stream_kernel<T, QQ, SS><<<blocks_for(a.g.n, b), b, 0, s>>>(a);           \
+        constexpr int b = G > 1 ? 256 : (swap_max_threads<T, QQ>() < 256 ? swap_max_threads<T, QQ>() : 256); \
+        swap_stream_kernel<T, QQ, SS, G><<<dim3(blocks_for(a.g.n, b), G), b, 0, s>>>(a); \
     }
     LBM_QS_DISPATCH(Q, soa, CALL);
 #undef CALL
