@@ -20,8 +20,16 @@ static cudaError_t launch_one(int block, bool staged, const StepArgs<T>& a, cuda
         }
     }
     const int b = block > max_threads<T, Q>() ? max_threads<T, Q>() : block;
-    step_kernel<T, Q, MODEL, SOA, LOAD, STORE><<<(a.end - a.first + b - 1) / b, b, 0, s>>>(a);
-    return cudaGetLastError();
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)((a.end - a.first + b - 1) / b));
+    cfg.blockDim = dim3((unsigned)b);
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = a.pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, step_kernel<T, Q, MODEL, SOA, LOAD, STORE>, a);
 }
 
 template <class T, int Q, int MODEL, bool SOA>

@@ -48,6 +48,7 @@ struct StepArgs {
     const unsigned long long* mask;
     Geo g;
     int first, end;   // the step kernel updates the cells [first, end): the whole box, or some x-layers (slab overlap)
+    int pdl;          // host side: launch with programmatic stream serialisation (see step_kernel)
     Rates<T> rt;
     T wterm[27];  // w_k
     // offsets filled on the host per launch (make_args) so that the kernels add one uniform
@@ -244,8 +245,15 @@ template <class T, int Q, int MODEL, bool SOA, int LOAD, int STORE>
 __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_kernel(const StepArgs<T> a)
 {
     constexpr bool SHIFT = sizeof(T) == 4;
+    // Programmatic dependent launch: the next step kernel of the stream may be scheduled as soon as
+    // every block of this one has started, and runs its prologue (cell codes and link masks, which
+    // no step kernel writes) while this grid drains; it touches populations only after
+    // griddepcontrol.wait, i.e. once this grid has completed and its stores are visible.  Without
+    // the launch attribute both instructions do nothing.
+    asm volatile("griddepcontrol.launch_dependents;");
     const int i = a.first + blockIdx.x * blockDim.x + threadIdx.x;
     const CellState cs = cell_state(a.code, a.mask, i, a.end);
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (!cs.active) {  // solid cells hold no populations
         // ... but when the other array is written (two-population), a warp that straddles a wall
         // fills the wall cells' slots too: a partially written 32 B sector that is not in L2 costs

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -66,6 +67,7 @@ struct lbm_ctx {
     // CUDA-graph replay of lbm_step for launch-bound lattices (see step_graphed)
     int graph_mode;             // LBM_GRAPH_AUTO / OFF / ON
     cudaGraphExec_t graph_exec; // GRAPH_STEPS steps starting from graph_sto with pop[0] == graph_pop0
+    int pdl;                     // programmatic dependent launch of the step kernels (LBM_PDL=0 in the environment turns it off)
     int range_first, range_end;  // cells the next step launch covers (0, 0 = all); lbm_step_begin / lbm_step_end
     bool mid_step;               // between lbm_step_begin and lbm_step_end
     cudaStream_t cap_stream;    // private stream the capture runs on (the context stream may be the
@@ -138,6 +140,7 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
     a.code = c->code;
     a.mask = c->mask;
     a.g = c->g;
+    a.pdl = c->pdl;
     a.first = c->range_first;
     a.end = c->range_end > 0 ? c->range_end : c->g.n;
     a.rt.omega = (T)c->omega;
@@ -373,6 +376,7 @@ lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme
     c->pop_elems = c->soa ? (size_t)c->g.stride * c->Q : (size_t)c->g.n * c->Q;
     c->alloc = g_alloc; c->free_fn = g_free; c->stream = g_stream;
     c->variant = V_DEFAULT;
+    { const char* e = getenv("LBM_PDL"); c->pdl = !(e && e[0] == '0'); }
     c->block = 128;
     c->n_fluid = c->g.n;
     lattice_tables(c->Q, c->c, c->opp, c->w);
