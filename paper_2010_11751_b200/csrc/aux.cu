@@ -168,14 +168,24 @@ template <class T>
 cudaError_t aux_swap_stream(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s)
 {
     constexpr int G = swap_groups<T>();
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cudaLaunchConfig_t cfg = {};
+    cfg.stream = s;
+    cfg.attrs = attr;
+    cfg.numAttrs = a.pdl ? 1 : 0;
+    cudaError_t e = cudaSuccess;
 #define CALL(QQ, SS)                                                                   \
     {                                                                                  \
         constexpr int b = G > 1 ? 256 : (swap_max_threads<T, QQ>() < 256 ? swap_max_threads<T, QQ>() : 256); \
-        swap_stream_kernel<T, QQ, SS, G><<<dim3(blocks_for(a.g.n, b), G), b, 0, s>>>(a); \
+        cfg.gridDim = dim3(blocks_for(a.g.n, b), G);                                   \
+        cfg.blockDim = dim3(b);                                                        \
+        e = cudaLaunchKernelEx(&cfg, swap_stream_kernel<T, QQ, SS, G>, a);             \
     }
     LBM_QS_DISPATCH(Q, soa, CALL);
 #undef CALL
-    return cudaGetLastError();
+    return e;
 }
 
 template <class T>

@@ -410,8 +410,10 @@ template <class T, int Q, bool SOA, int G>
 __global__ void __launch_bounds__(G == 1 ? swap_max_threads<T, Q>() : 256, G == 1 ? swap_min_blocks<T, Q>() : (sizeof(T) == 8 ? 5 : 6))
 swap_stream_kernel(const StepArgs<T> a)
 {
+    asm volatile("griddepcontrol.launch_dependents;");   // see step_kernel
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     if (!cs.active) return;
     static_for<G>([&](auto gc) {
         if (blockIdx.y == (unsigned)gc) swap_pairs<T, Q, SOA, G, gc>(a, i, cs);
