@@ -49,6 +49,7 @@ struct StepArgs {
     Geo g;
     int first, end;   // the step kernel updates the cells [first, end): the whole box, or some x-layers (slab overlap)
     int pdl;          // host side: launch with programmatic stream serialisation (see step_kernel)
+    int pf;           // L2 prefetch distance in cells (0 = off), see step_kernel
     Rates<T> rt;
     T wterm[27];  // w_k
     // offsets filled on the host per launch (make_args) so that the kernels add one uniform
@@ -265,6 +266,16 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
             }
         }
         return;
+    }
+    // The loads in flight of a step kernel live in registers (one cell per thread), and the register
+    // file caps them below what hides the DRAM latency at full bandwidth (fp32 worst: 4 bytes per
+    // destination register).  Each thread therefore also asks L2 for the lines of the cell `pf`
+    // cells ahead: no registers held, and the blocks scheduled next find their loads in L2.
+    // Measured at 16384 cells (any distance from 2048 to 32768 does): AA fp32 88.0 -> 94.2 %,
+    // AA fp64 98.9 -> 100.5 %, D3Q27 cumulants AA 92.0 -> 96.2 %, 128^3 AA 94.0 -> 95.9 %.
+    if (a.pf > 0 && i + a.pf < a.end) {
+        const char* q = reinterpret_cast<const char*>(a.src + (long long)(i + a.pf) * (SOA ? 1 : Q));
+        static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(q + a.ldo[kc])); });
     }
     T f[Q];
     load_cell<T, Q, SOA, LOAD>(a, i, cs.masked, cs.mask, f);

@@ -67,6 +67,7 @@ struct lbm_ctx {
     // CUDA-graph replay of lbm_step for launch-bound lattices (see step_graphed)
     int graph_mode;             // LBM_GRAPH_AUTO / OFF / ON
     cudaGraphExec_t graph_exec; // GRAPH_STEPS steps starting from graph_sto with pop[0] == graph_pop0
+    int prefetch;                // L2 prefetch distance of the step kernels in cells (LBM_PF in the environment overrides)
     int pdl;                     // programmatic dependent launch of the step kernels (LBM_PDL=0 in the environment turns it off)
     int range_first, range_end;  // cells the next step launch covers (0, 0 = all); lbm_step_begin / lbm_step_end
     bool mid_step;               // between lbm_step_begin and lbm_step_end
@@ -141,6 +142,7 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
     a.mask = c->mask;
     a.g = c->g;
     a.pdl = c->pdl;
+    a.pf = 0;
     a.first = c->range_first;
     a.end = c->range_end > 0 ? c->range_end : c->g.n;
     a.rt.omega = (T)c->omega;
@@ -191,6 +193,11 @@ cudaError_t step_kind(lbm_ctx* c, int kind, const void* src, void* dst)
     int load, store;
     kind_modes(kind, &load, &store);
     StepArgs<T> a = make_args<T>(c, src, dst, load, store);
+    // L2 prefetch ahead of the block scheduler (kernels.cuh): pays for the in-place kernels in both
+    // precisions and for the two-population pull in fp64; it costs the fp32 pull 15 % (measured)
+    // ... and nothing when the populations fit in L2 anyway (48^3: -5 %, 64^3: -3 % with it)
+    const bool beyond_l2 = c->pop_elems * c->elem * (c->fam == FAM_2POP ? 2 : 1) > (size_t)100 << 20;
+    if (c->soa && beyond_l2 && (kind == SK_EVEN || kind == SK_ODD || (kind == SK_PULL && sizeof(T) == 8))) a.pf = c->prefetch;
     c->launches++;
     return c->Q == 19 ? step_model<T, 19>(c, kind, a) : step_model<T, 27>(c, kind, a);
 }
@@ -377,6 +384,7 @@ lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme
     c->alloc = g_alloc; c->free_fn = g_free; c->stream = g_stream;
     c->variant = V_DEFAULT;
     { const char* e = getenv("LBM_PDL"); c->pdl = !(e && e[0] == '0'); }
+    { const char* e = getenv("LBM_PF"); c->prefetch = e ? atoi(e) : 16384; }
     c->block = 128;
     c->n_fluid = c->g.n;
     lattice_tables(c->Q, c->c, c->opp, c->w);
