@@ -427,7 +427,19 @@ swap_stream_kernel(const StepArgs<T> a)
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (!cs.active) return;
     static_for<G>([&](auto gc) {
-        if (blockIdx.y == (unsigned)gc) swap_pairs<T, Q, SOA, G, gc>(a, i, cs);
+        if (blockIdx.y == (unsigned)gc) {
+            if (a.pf > 0 && i + a.pf < a.g.n) {  // L2 prefetch ahead of the block scheduler, see step_kernel
+                using L = Lat<Q>;
+                static_for<L::NH>([&](auto kc) {
+                    constexpr int k = kc, kb = L::opp(k);
+                    if constexpr (k % G == gc) {
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(a.dst + slot<SOA, Q>(a.g, kb, (long long)i + a.pf)));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(a.dst + slot<SOA, Q>(a.g, k, (long long)i + a.pf + offset<Q, k>(a.g))));
+                    }
+                });
+            }
+            swap_pairs<T, Q, SOA, G, gc>(a, i, cs);
+        }
     });
 }
 

@@ -255,8 +255,16 @@ int one_step(lbm_ctx* c)
         }
     } else {
         CK(step_kind(c, SK_EVEN, c->pop[0], c->pop[0]));  // pass 1: collide into opposite slots
-        if (c->dtype == LBM_F64) CK(aux_swap_stream<double>(c->Q, c->soa, make_args<double>(c, c->pop[0], c->pop[0]), c->stream));
-        else CK(aux_swap_stream<float>(c->Q, c->soa, make_args<float>(c, c->pop[0], c->pop[0]), c->stream));
+        const bool pf = c->soa && c->pop_elems * c->elem > (size_t)100 << 20;  // as in step_kind
+        if (c->dtype == LBM_F64) {
+            StepArgs<double> a = make_args<double>(c, c->pop[0], c->pop[0]);
+            if (pf) a.pf = c->prefetch;
+            CK(aux_swap_stream<double>(c->Q, c->soa, a, c->stream));
+        } else {
+            StepArgs<float> a = make_args<float>(c, c->pop[0], c->pop[0]);
+            if (pf) a.pf = c->prefetch;
+            CK(aux_swap_stream<float>(c->Q, c->soa, a, c->stream));
+        }
         c->launches++;
     }
     c->steps++;
