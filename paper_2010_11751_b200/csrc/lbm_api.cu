@@ -143,6 +143,7 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
     a.g = c->g;
     a.pdl = c->pdl;
     a.pf = 0;
+    a.pf_strided = 0;
     a.first = c->range_first;
     a.end = c->range_end > 0 ? c->range_end : c->g.n;
     a.rt.omega = (T)c->omega;
@@ -193,11 +194,14 @@ cudaError_t step_kind(lbm_ctx* c, int kind, const void* src, void* dst)
     int load, store;
     kind_modes(kind, &load, &store);
     StepArgs<T> a = make_args<T>(c, src, dst, load, store);
-    // L2 prefetch ahead of the block scheduler (kernels.cuh): pays for the in-place kernels in both
-    // precisions and for the two-population pull in fp64; it costs the fp32 pull 15 % (measured)
-    // ... and nothing when the populations fit in L2 anyway (48^3: -5 %, 64^3: -3 % with it)
+    // L2 prefetch ahead of the block scheduler (kernels.cuh) for the kernels of the steady state: per
+    // thread in fp64, one warp in 32 with a line per lane in fp32; nothing when the populations fit
+    // in L2 anyway (48^3: -5 %, 64^3: -3 % with it).  LBM_PF=<cells> overrides the distance, 0 = off.
     const bool beyond_l2 = c->pop_elems * c->elem * (c->fam == FAM_2POP ? 2 : 1) > (size_t)100 << 20;
-    if (c->soa && beyond_l2 && (kind == SK_EVEN || kind == SK_ODD || (kind == SK_PULL && sizeof(T) == 8))) a.pf = c->prefetch;
+    if (c->soa && beyond_l2 && (kind == SK_EVEN || kind == SK_ODD || kind == SK_PULL)) {
+        a.pf_strided = sizeof(T) == 4;
+        a.pf = c->prefetch >= 0 ? c->prefetch : (sizeof(T) == 4 ? 65536 : 16384);
+    }
     c->launches++;
     return c->Q == 19 ? step_model<T, 19>(c, kind, a) : step_model<T, 27>(c, kind, a);
 }
@@ -258,11 +262,11 @@ int one_step(lbm_ctx* c)
         const bool pf = c->soa && c->pop_elems * c->elem > (size_t)100 << 20;  // as in step_kind
         if (c->dtype == LBM_F64) {
             StepArgs<double> a = make_args<double>(c, c->pop[0], c->pop[0]);
-            if (pf) a.pf = c->prefetch;
+            if (pf) a.pf = c->prefetch >= 0 ? c->prefetch : 16384;
             CK(aux_swap_stream<double>(c->Q, c->soa, a, c->stream));
         } else {
             StepArgs<float> a = make_args<float>(c, c->pop[0], c->pop[0]);
-            if (pf) a.pf = c->prefetch;
+            if (pf) a.pf = c->prefetch >= 0 ? c->prefetch : 16384;
             CK(aux_swap_stream<float>(c->Q, c->soa, a, c->stream));
         }
         c->launches++;
@@ -392,7 +396,7 @@ lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme
     c->alloc = g_alloc; c->free_fn = g_free; c->stream = g_stream;
     c->variant = V_DEFAULT;
     { const char* e = getenv("LBM_PDL"); c->pdl = !(e && e[0] == '0'); }
-    { const char* e = getenv("LBM_PF"); c->prefetch = e ? atoi(e) : 16384; }
+    { const char* e = getenv("LBM_PF"); c->prefetch = e ? atoi(e) : -1; }  // -1 = the tuned distances
     c->block = 128;
     c->n_fluid = c->g.n;
     lattice_tables(c->Q, c->c, c->opp, c->w);
