@@ -159,6 +159,11 @@ enum { LBM_GRAPH_AUTO = 0, LBM_GRAPH_OFF = 1, LBM_GRAPH_ON = 2 };
 int lbm_set_graph(lbm_t* ctx, int mode);
 long long lbm_graph_replays(const lbm_t* ctx);
 
+/* Tuning knobs read from the environment by lbm_create (results never depend on them):
+ *   LBM_PF=<cells>  distance of the L2 prefetch the step kernels issue ahead of the block scheduler
+ *                   (default 16384 cells in fp64, 65536 in fp32; 0 = off; only lattices beyond L2);
+ *   LBM_PDL=0       no programmatic dependent launch of the step kernels. */
+
 const char* lbm_last_error(void);
 const char* lbm_version(void);
 
