@@ -266,7 +266,8 @@ def run_gpu(args):
     g.macroscopic_device(out_rho_d.data_ptr(), out_u_d.data_ptr())
     g.kinetic_energy()
     sampler = ClockSampler(local_rank)
-    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(5)]
+    e_d = torch.zeros(1, dtype=torch.float64, device=dev)
     barrier()
     sampler.start()
     l0 = g.kernel_launches
@@ -275,14 +276,17 @@ def run_gpu(args):
     ev[1].record()
     g.macroscopic_device(out_rho_d.data_ptr(), out_u_d.data_ptr())   # a9
     ev[2].record()
-    energy = g.kinetic_energy()                 # a10 (synchronises; 8 B to the host)
+    g.kinetic_energy_device(e_d.data_ptr())     # a10 on the device (three kernels)
+    ev[4].record()
+    energy = g.kinetic_energy()                 # a10 again through the host call (synchronises; 8 B to the host)
     ev[3].record()
     barrier()
     launches = g.kernel_launches - l0
     ms_total = ev[0].elapsed_time(ev[3])
     ms_steps = ev[0].elapsed_time(ev[1])
     ms_macro = ev[1].elapsed_time(ev[2])
-    ms_energy = ev[2].elapsed_time(ev[3])
+    ms_energy = ev[2].elapsed_time(ev[4])
+    assert abs(float(e_d.item()) - energy) == 0.0   # fixed reduction tree: bitwise repeatable
     assert np.isfinite(energy), "simulation blew up"
 
     # ---- end-to-end leg: host buffers in, host buffers out, copies inside the timed region ----
@@ -328,7 +332,7 @@ def run_gpu(args):
             "step": {"ms": step_ms, "mlups": nfluid / step_ms / 1e3, "gbs": achieved},
             "macroscopic": {"ms": ms_macro, "gbs": nfluid * (Q + 4) * s / (ms_macro * 1e-3) / 1e9},
             "kinetic_energy": {"ms": ms_energy, "gbs": nfluid * Q * s / (ms_energy * 1e-3) / 1e9,
-                               "note": "includes the 8-byte D2H copy and stream sync"},
+                               "note": "lbm_kinetic_energy_device: reduce kernel + two summing stages"},
         },
         "e2e": {"value": units_g / (ms_e2e_g * 1e-3) / 1e6, "unit": UNIT,
                 "h2d_bytes_per_step": 4 * N * s / K, "d2h_bytes_per_step": (4 * N * s + 8) / K,

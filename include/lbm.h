@@ -95,6 +95,8 @@ int lbm_macroscopic_device(lbm_t* ctx, void* rho_dev, void* u_dev);
 /* E = sum over fluid cells of 1/2 rho |u|^2 (R19), accumulated in double with a fixed reduction
  * tree (bitwise repeatable); synchronises. */
 int lbm_kinetic_energy(lbm_t* ctx, double* e);
+/* Same into one double in DEVICE memory; asynchronous on the stream. */
+int lbm_kinetic_energy_device(lbm_t* ctx, double* e_dev);
 
 /* Pre-collision populations at the current time, canonical [Q][N] order, context dtype, host. */
 int lbm_get_populations(lbm_t* ctx, void* f);

@@ -577,18 +577,25 @@ int lbm_macroscopic(lbm_t* c, void* rho, void* u)
     return LBM_OK;
 }
 
-int lbm_kinetic_energy(lbm_t* c, double* e)
+int lbm_kinetic_energy_device(lbm_t* c, double* e_dev)
 {
-    if (!c || !e) { set_err("null argument"); return LBM_E_ARG; }
+    if (!c || !e_dev) { set_err("null argument"); return LBM_E_ARG; }
     if (c->mid_step) { set_err("export between lbm_step_begin and lbm_step_end"); return LBM_E_STATE; }
     if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
     if (c->dtype == LBM_F64)
         CK(aux_energy<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr, load_mode(c)), c->partial,
-                              c->n_partial, c->e_dev, c->stream));
+                              c->n_partial, e_dev, c->stream));
     else
         CK(aux_energy<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr, load_mode(c)), c->partial,
-                             c->n_partial, c->e_dev, c->stream));
+                             c->n_partial, e_dev, c->stream));
     c->launches += 3;
+    return LBM_OK;
+}
+
+int lbm_kinetic_energy(lbm_t* c, double* e)
+{
+    if (!c || !e) { set_err("null argument"); return LBM_E_ARG; }
+    if (int rc = lbm_kinetic_energy_device(c, c->e_dev)) return rc;
     CK(cudaMemcpyAsync(e, c->e_dev, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
     return LBM_OK;

@@ -87,6 +87,10 @@ def test_config1_cavity32_bgk_2pop_fp64(Lbm, oracle):
     eg, eo = g.kinetic_energy(), o.kinetic_energy()
     assert abs(eg - eo) <= 1e-12 * max(1.0, abs(eo))
     assert eg == g.kinetic_energy()  # fixed reduction tree: bitwise repeatable
+    import torch
+    e_d = torch.zeros(1, dtype=torch.float64, device="cuda")
+    g.kinetic_energy_device(e_d.data_ptr())
+    assert float(e_d.item()) == eg
 
 
 @pytest.mark.parametrize("variant", ["generic_push", "generic_pull"])
