@@ -167,7 +167,6 @@ cudaError_t aux_insert_plane(int Q, bool soa, T* pop, const uint8_t* code, const
 template <class T>
 cudaError_t aux_swap_stream(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s)
 {
-    constexpr int G = swap_groups<T>();
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
@@ -178,6 +177,7 @@ cudaError_t aux_swap_stream(int Q, bool soa, const StepArgs<T>& a, cudaStream_t 
     cudaError_t e = cudaSuccess;
 #define CALL(QQ, SS)                                                                   \
     {                                                                                  \
+        constexpr int G = swap_groups<T, QQ>();                                        \
         constexpr int b = G > 1 ? 256 : (swap_max_threads<T, QQ>() < 256 ? swap_max_threads<T, QQ>() : 256); \
         cfg.gridDim = dim3(blocks_for(a.g.n, b), G);                                   \
         cfg.blockDim = dim3(b);                                                        \

@@ -374,8 +374,8 @@ constexpr int swap_min_blocks() { return (sizeof(T) == 8 && Q == 27) ? LBM_SWAP_
 #ifndef LBM_SWAP_G_F32
 #define LBM_SWAP_G_F32 1
 #endif
-template <class T>
-constexpr int swap_groups() { return sizeof(T) == 8 ? LBM_SWAP_G_F64 : LBM_SWAP_G_F32; }
+template <class T, int Q>
+constexpr int swap_groups() { return sizeof(T) == 8 ? LBM_SWAP_G_F64 : (Q == 27 ? 2 : LBM_SWAP_G_F32); }  // fp32 D3Q27: 82.5 -> 86.6 %
 template <class T, int Q, bool SOA, int G, int GI>
 __device__ __forceinline__ void swap_pairs(const StepArgs<T>& a, int i, const CellState& cs)
 {
