@@ -19,6 +19,24 @@ def test_bytes_per_update():
     assert bench.bytes_per_update(27, "f64", "AA_AOS") == 432
 
 
+def test_roofline_arithmetic_reproduces_the_papers_table3():
+    """tests/golden/paper_table3_peak_fractions.txt: the paper's own MLUPS and "% of peak" for three GPUs
+    (Table 3, Eq 16).  bench.py's bytes per update and MLUPS -> fraction arithmetic
+    must give back the printed percentages (they are rounded to integers)."""
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2010_11751_b200 import sweep
+    rows = [l.split("|") for l in open(os.path.join(ROOT, "tests", "golden", "paper_table3_peak_fractions.txt"))
+            if l.strip() and not l.startswith("#")]
+    assert len(rows) == 9
+    for gpu, bw, code, mlups, pct in rows:
+        scheme = "AA_SOA" if "AA" in code else "2POP_SOA"
+        bpu = bench.bytes_per_update(19, "f64", scheme)
+        assert bpu == sweep.bytes_per_update(19, "f64", scheme) == 2 * 19 * 8
+        frac = float(mlups) * 1e6 * bpu / (float(bw) * 1e9)
+        assert abs(100.0 * frac - float(pct)) <= 0.6, (gpu, code, 100.0 * frac, pct)
+
+
 _WORKER = r"""
 import os, sys
 sys.path.insert(0, %r)
