@@ -279,8 +279,11 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
     // 88.0 -> 95.2 %, 2-pop fp32 86.7 -> 90.6 %, cumulants AA fp32 82.7 -> 89.1 %, AA fp64 98.9 ->
     // 100.5 %, D3Q27 cumulants AA fp64 92.0 -> 96.2 %, 128^3 AA fp64 94.0 -> 95.9 %.
     if (a.pf > 0) {
+        // keep every prefetched address inside the arrays: a neighbour offset reaches at most one
+        // x-layer + one row + one cell beyond the target cell, so stay that far from both ends
+        const long long margin = (long long)a.g.ny * a.g.nz + a.g.nz + 1;
         if (!a.pf_strided) {
-            if (i + a.pf < a.end) {
+            if (i + a.pf >= margin && i + a.pf + margin < a.g.n && i + a.pf < a.end) {
                 const char* q = reinterpret_cast<const char*>(a.src + (long long)(i + a.pf) * (SOA ? 1 : Q));
                 static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(q + a.ldo[kc])); });
             }
@@ -288,7 +291,7 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
             constexpr int CPL = 128 / sizeof(T);   // cells per line
             const int lane = threadIdx.x & 31;
             const long long tgt = (long long)(i - lane) + a.pf + (long long)lane * CPL;
-            if ((((i - a.first) >> 5) % CPL) == 0 && tgt + CPL < a.end) {
+            if ((((i - a.first) >> 5) % CPL) == 0 && tgt >= margin && tgt + CPL + margin < a.g.n && tgt + CPL < a.end) {
                 const char* q = reinterpret_cast<const char*>(a.src + tgt);
                 static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(q + a.ldo[kc])); });
             }
@@ -445,7 +448,7 @@ swap_stream_kernel(const StepArgs<T> a)
     if (!cs.active) return;
     static_for<G>([&](auto gc) {
         if (blockIdx.y == (unsigned)gc) {
-            if (a.pf > 0 && i + a.pf < a.g.n) {  // L2 prefetch ahead of the block scheduler, see step_kernel
+            if (a.pf > 0 && (long long)i + a.pf + (long long)a.g.ny * a.g.nz + a.g.nz + 1 < a.g.n) {  // L2 prefetch, see step_kernel (offsets of the half set point forward only)
                 using L = Lat<Q>;
                 static_for<L::NH>([&](auto kc) {
                     constexpr int k = kc, kb = L::opp(k);
