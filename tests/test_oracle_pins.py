@@ -593,6 +593,54 @@ def test_p3_shear_wave_config2_omega(oracle):
     assert abs(ratio - np.exp(-nu * (2 * np.pi / 128) ** 2 * 1000)) < 5e-4
 
 
+# ------------------------------------------------------------------ R19: kinetic energy, absolute value
+
+def test_kinetic_energy_absolute_shear_wave(oracle):
+    """E = sum_fluid 1/2 rho |u|^2 (R19).  On the 1 x 128 x 1 shear wave at t = 0 (rho = 1,
+    u_x = 0.01 sin(2 pi y/128)) the sum is closed form: 1/2 * 1 * 0.01^2 * sum_y sin^2 = 1/2 * 1e-4 * 64
+    = 3.2e-3 exactly.  Pins the 1/2, the square and the density factor (a constant-factor mistake
+    passes the ratio test of P3 but not this one)."""
+    ny = 128
+    for Q in LATTICES:
+        rho, u = inputs.shear_wave(1, ny, 1)
+        o = oracle.Oracle(1, ny, 1, Q, "BGK_W2", 1.3)
+        o.set_flags(np.zeros(ny, dtype=np.uint8))
+        o.init_equilibrium(rho, u)
+        assert abs(o.kinetic_energy() - 3.2e-3) < 1e-15
+        # twice the density at the same velocity doubles the energy (rho enters linearly, not squared)
+        o.init_equilibrium(2.0 * rho, u)
+        assert abs(o.kinetic_energy() - 6.4e-3) < 2e-15
+        # twice the velocity quadruples it
+        o.init_equilibrium(rho, 2.0 * u)
+        assert abs(o.kinetic_energy() - 12.8e-3) < 4e-15
+
+
+def test_kinetic_energy_hand_sum_skips_solid_cells(oracle):
+    """Three cells in a row, hand-made populations.  Cell 0: rest 1, f(+1,0,0) = 1/2: rho = 3/2,
+    rho u = (1/2,0,0), E = 1/2 * (1/2)^2 / (3/2) = 1/12.  Cell 1: WALL (or MOVING), every slot holding
+    garbage: contributes nothing (fluid-only restriction, R19; PAPER.md:L94 solid cells carry no
+    populations).  Cell 2: rest 2, f(0,-1,0) = f(0,0,+1) = 1/2: rho = 3, rho u = (0,-1/2,1/2),
+    E = 1/2 * (1/4 + 1/4) / 3 = 1/12.  Total 1/6."""
+    for Q in LATTICES:
+        c, t, opp, _ = oracle.lattice(Q)
+        k_of = {tuple(v): k for k, v in enumerate(c)}
+        for solid in (inputs.WALL, inputs.MOVING):
+            f = np.zeros((Q, 3))
+            f[k_of[(0, 0, 0)], 0] = 1.0
+            f[k_of[(1, 0, 0)], 0] = 0.5
+            f[:, 1] = 1.0e6                      # garbage in the solid cell's slots
+            f[k_of[(0, 0, 0)], 2] = 2.0
+            f[k_of[(0, -1, 0)], 2] = 0.5
+            f[k_of[(0, 0, 1)], 2] = 0.5
+            o = oracle.Oracle(1, 3, 1, Q, "BGK_W2", 1.0)
+            o.set_flags(np.array([inputs.FLUID, solid, inputs.FLUID], dtype=np.uint8), (0.3, 0.0, 0.0))
+            o.set_populations(f)
+            assert abs(o.kinetic_energy() - 1.0 / 6.0) < 1e-15
+            rho, u = o.macroscopic()
+            assert abs(rho[0] - 1.5) < 1e-15 and abs(u[0][0] - 1.0 / 3.0) < 1e-15
+            assert abs(rho[2] - 3.0) < 1e-15 and abs(u[1][2] + 1.0 / 6.0) < 1e-15 and abs(u[2][2] - 1.0 / 6.0) < 1e-15
+
+
 # ------------------------------------------------------------------ P4: Poiseuille between bounce-back walls
 
 @pytest.mark.parametrize("model,lam", [("TRT", 3 / 16), ("TRT", 1 / 4), ("BGK_W2", None)])
