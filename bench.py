@@ -17,7 +17,6 @@ import argparse
 import json
 import os
 import sys
-import threading
 import time
 
 import numpy as np
@@ -60,52 +59,7 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-class ClockSampler:
-    """SM clock and throttle reasons sampled with NVML while the timed regions run."""
-
-    def __init__(self, index):
-        self.samples, self.reasons, self.max_mhz, self._stop = [], set(), None, threading.Event()
-        self._thread = None
-        try:
-            import pynvml
-            pynvml.nvmlInit()
-            self.nv = pynvml
-            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
-            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
-        except Exception:
-            self.nv = None
-
-    def _loop(self):
-        nv = self.nv
-        names = {
-            nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
-            nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
-            nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
-            nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
-            nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake",
-        }
-        while not self._stop.is_set():
-            try:
-                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
-                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
-                for bit, name in names.items():
-                    if mask & bit:
-                        self.reasons.add(name)
-            except Exception:
-                pass
-            time.sleep(0.02)
-
-    def start(self):
-        if self.nv is not None:
-            self._thread = threading.Thread(target=self._loop, daemon=True)
-            self._thread.start()
-
-    def stop(self):
-        self._stop.set()
-        if self._thread is not None:
-            self._thread.join()
-        med = float(np.median(self.samples)) if self.samples else None
-        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": len(self.samples)}
+from paper_2010_11751_b200.clocks import ClockSampler  # noqa: E402
 
 
 def dist_setup(n_gpus):
@@ -149,6 +103,15 @@ def traffic_from_profiles(workload, kernel):
     return None
 
 
+def set_oracle_threads(n):
+    """OpenMP thread count of the oracle library (libgomp is already loaded by it); n <= 0 = all cores"""
+    import ctypes
+    from oracle import lbm_oracle
+    lbm_oracle.lib()
+    gomp = ctypes.CDLL("libgomp.so.1")
+    gomp.omp_set_num_threads(int(n) if n > 0 else (os.cpu_count() or 1))
+
+
 def oracle_sample_time(n, Q, model, re, steps, warm=1):
     """seconds per oracle step on an n^3 cavity of the workload's recipe (bounded sample)"""
     from oracle import lbm_oracle  # bench.py's cpu_baseline / --impl reference legs may use the oracle
@@ -167,14 +130,43 @@ def oracle_sample_time(n, Q, model, re, steps, warm=1):
     return dt / steps, int((fl == 0).sum()), lbm_oracle.num_threads()
 
 
-def cpu_baseline(workload, budget_s=15.0):
+def oracle_sample_size(n, Q, model, re, budget_s, min_steps=3):
+    """largest cavity edge <= min(n, 256) of which `min_steps` oracle steps fit into budget_s, from
+    the rate of a 64^3 probe (from there on the oracle's rate per cell hardly depends on the size)"""
+    probe = 64 if n >= 64 else 32
+    t32, nf32, _ = oracle_sample_time(probe, Q, model, re, 2)
+    per_cell = t32 / nf32
+    for ns in (n, 256, 192, 128, 96, 64, 48, 32):
+        if ns <= min(n, 256) and per_cell * (ns - 2) ** 3 * (min_steps + 1) <= budget_s:
+            return ns
+    return 32
+
+
+def cpu_baseline(workload, budget_s=20.0):
+    """the oracle as it stands on the host cores: all cores on a bounded sample of the workload (its own
+    lattice when 3 steps of it fit the budget, else a smaller cavity of the same recipe), plus the
+    single-thread rate at 32^3 and 128^3 that SURVEY 8(d) asks for"""
     n, Q, model, scheme, dtype, re = WORKLOADS[workload]
-    ns = min(n, 128 if Q == 19 and model in ("BGK_W2", "TRT", "REG") else 48)
-    t1, nfluid, threads = oracle_sample_time(ns, Q, model, re, 2)
-    steps = int(max(2, min(400, budget_s / max(t1, 1e-6))))
+    set_oracle_threads(0)
+    ns = oracle_sample_size(n, Q, model, re, budget_s)
+    t1, nfluid, threads = oracle_sample_time(ns, Q, model, re, 1)
+    steps = int(max(3, min(400, budget_s / max(t1, 1e-6))))
     t, nfluid, threads = oracle_sample_time(ns, Q, model, re, steps)
-    return {"value": nfluid / t / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
-            "sample": "%d^3 lid cavity of the same recipe (%s D3Q%d, fp64), %d oracle steps, OpenMP over x" % (ns, model, Q, steps)}
+    out = {"value": nfluid / t / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle",
+           "sample": "%d^3 lid cavity of the same recipe (%s D3Q%d, fp64)%s, %d oracle steps, OpenMP over x"
+                     % (ns, model, Q, "" if ns == n else " standing in for the %d^3 workload" % n, steps)}
+    set_oracle_threads(1)
+    single = {}
+    for m in (32, 128):
+        t32, nf32, _ = oracle_sample_time(32, Q, model, re, 1, warm=0)
+        if m == 128 and t32 / nf32 * 126 ** 3 * 2 > 30.0:     # generic-matrix models: 128^3 on one thread takes minutes
+            single["128^3"] = None
+            continue
+        ts, nf, _ = oracle_sample_time(m, Q, model, re, 10 if m == 32 else 1, warm=1 if m == 32 else 0)
+        single["%d^3" % m] = nf / ts / 1e6
+    set_oracle_threads(0)
+    out["single_thread_mlups"] = single
+    return out
 
 
 def run_reference(args):
@@ -182,14 +174,12 @@ def run_reference(args):
     if int(os.environ.get("RANK", "0")) != 0:
         return
     n, Q, model, scheme, dtype, re = WORKLOADS[args.workload]
-    ns = min(n, 128 if Q == 19 and model in ("BGK_W2", "TRT", "REG") else 48)
-    t1, nfluid, threads = oracle_sample_time(ns, Q, model, re, 2)
-    while ns > 32 and t1 * (args.steps + args.warmup) > 150.0:  # keep the whole run within minutes
-        ns //= 2
-        t1, nfluid, threads = oracle_sample_time(ns, Q, model, re, 2)
+    # every step = one oracle time step over the sample; the whole run must end within minutes
+    ns = oracle_sample_size(n, Q, model, re, 150.0, min_steps=args.steps + args.warmup)
     t, nfluid, threads = oracle_sample_time(ns, Q, model, re, args.steps, warm=args.warmup)
     value = nfluid / t / 1e6
-    sample = "%d^3 lid cavity of the same recipe, every step one oracle time step over it" % ns
+    sample = "%d^3 lid cavity of the same recipe%s, every step one oracle time step over it" % (
+        ns, "" if ns == n else " (bounded sample of the %d^3 workload)" % n)
     line = {
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": t * 1e3, "higher_is_better": True, "scaling": "weak",
@@ -443,12 +433,18 @@ def main():
     ap.add_argument("--steps", type=int, default=1000)
     ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="target", choices=sorted(WORKLOADS))
+    ap.add_argument("--workload", default="target", choices=sorted(WORKLOADS) + ["case"])
+    ap.add_argument("--case", default=None,
+                    help="any other case N,Q,MODEL,SCHEME,DTYPE[,RE], e.g. 256,19,BGK_W2,2POP_AOS,f64 (overrides --workload)")
     ap.add_argument("--variant", default=None, help="step-kernel variant (binding.VARIANTS), default = library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
                     help="replicas (default): N independent lattices; slab: one lattice cut along x with a halo exchange")
     args = ap.parse_args()
+    if args.case:
+        p = args.case.split(",")
+        WORKLOADS["case"] = (int(p[0]), int(p[1]), p[2], p[3], p[4], int(p[5]) if len(p) > 5 else 1000)
+        args.workload = "case"
     if args.impl == "reference":
         run_reference(args)
     elif args.decomp == "slab":

@@ -25,6 +25,7 @@ import sys
 import numpy as np
 
 from . import inputs
+from .clocks import ClockSampler
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 ALL_MODELS = ["BGK_W2", "BGK_NW4", "TRT", "RM", "HM", "CM", "CHM", "K", "RR", "REG"]
@@ -59,6 +60,11 @@ def groups():
     # fixed omega (config 1's): Re = 1000 would push omega to 1.998 at N = 16, where the seeded noise blows BGK up
     g["sizes"] = [case(n, model=m, scheme=s, omega=inputs.omega_from_re(32, 100)) for m in ("BGK_W2", "RR")
                   for s in ("2POP_SOA", "AA_SOA") for n in sizes]
+    # Fig 7 resolved where the L2 plateau and cliff are (PAPER.md:L484 steps N by 1): every 4th size from
+    # 48 to 128 plus sizes that are not multiples of 4, 8 or 32
+    fine = sorted(set(list(range(48, 129, 4)) + [50, 63, 65, 75, 81, 85, 90, 95, 99, 101, 110, 127, 129, 150, 200, 250, 255, 257, 300]))
+    g["sizes_fine"] = [case(n, model="BGK_W2", scheme=s, omega=inputs.omega_from_re(32, 100)) for s in ("2POP_SOA", "AA_SOA")
+                       for n in fine]
     g["rr400"] = [case(400, model="RR", scheme=s, re=10000, bulk=1.0) for s in ("2POP_SOA", "AA_SOA")]
     g["target"] = [case(256), case(256, scheme="AA_SOA")]
     g["blocks"] = [case(256, scheme=s, dtype=d, block=b) for d in ("f64", "f32") for s in ("2POP_SOA", "AA_SOA")
@@ -113,6 +119,9 @@ def run_case(c, steps, repeat, warmup):
             g.set_relaxation(c["bulk"], hi, hi)
         g.init_equilibrium_device(rho_d.data_ptr(), u_d.data_ptr())
         g.step(warmup)
+        torch.cuda.synchronize()
+        sampler = ClockSampler(torch.cuda.current_device())
+        sampler.start()
         times = []
         for _ in range(repeat):
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -121,8 +130,10 @@ def run_case(c, steps, repeat, warmup):
             e1.record()
             torch.cuda.synchronize()
             times.append(e0.elapsed_time(e1) / steps)
+        clocks = sampler.stop()
         energy = g.kinetic_energy()
         nfluid = g.num_fluid
+        dev_bytes = g.device_bytes
     finally:
         g.close()
     ms = float(np.median(times))
@@ -130,18 +141,21 @@ def run_case(c, steps, repeat, warmup):
     gbs = nfluid * bpu / (ms * 1e-3) / 1e9
     out = dict(c)
     out.update(ms_per_step=ms, mlups=nfluid / ms / 1e3, gbs=gbs, frac=gbs / peak_gbs(), bytes_per_update=bpu,
-               fluid_cells=int(nfluid), steps=steps, finite=bool(np.isfinite(energy)), kinetic_energy=energy)
+               fluid_cells=int(nfluid), steps=steps, finite=bool(np.isfinite(energy)), kinetic_energy=energy,
+               clocks=clocks, device_bytes=int(dev_bytes))
     return out
 
 
 def to_md(rows, title):
     lines = ["### %s" % title, "",
-             "| N | lattice | model | scheme | dtype | variant | block | ms/step | MLUPS (fluid) | GB/s (algorithmic) | of measured copy | finite |",
-             "|---|---|---|---|---|---|---|---|---|---|---|---|"]
+             "| N | lattice | model | scheme | dtype | variant | block | ms/step | MLUPS (fluid) | GB/s (algorithmic) | of measured copy | finite | SM MHz (median / max) | throttle reasons | clock samples |",
+             "|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|"]
     for r in rows:
-        lines.append("| %d | D3Q%d | %s | %s | %s | %s | %s | %.4f | %.0f | %.0f | %.1f %% | %s |" % (
+        ck = r.get("clocks") or {}
+        lines.append("| %d | D3Q%d | %s | %s | %s | %s | %s | %.4f | %.0f | %.0f | %.1f %% | %s | %s / %s | %s | %s |" % (
             r["n"], r["Q"], r["model"], r["scheme"], r["dtype"], r["variant"] or "default", r["block"] or "default", r["ms_per_step"], r["mlups"],
-            r["gbs"], 100 * r["frac"], "yes" if r["finite"] else "NO"))
+            r["gbs"], 100 * r["frac"], "yes" if r["finite"] else "NO", ck.get("sm_mhz"), ck.get("sm_max_mhz"),
+            ",".join(ck.get("reasons") or []) or "none", ck.get("samples")))
     return "\n".join(lines) + "\n"
 
 

@@ -66,7 +66,7 @@ def make_gpu(Lbm, n, Q, model, scheme, dtype, omega, fl, uw, rho, u, bulk_one=Tr
     return g
 
 
-def subbox_error(g, oracle, n, Q, model, dtype, omega, fl, uw, rho, u, steps, b=6, bulk_one=True):
+def subbox_error(g, oracle, n, Q, model, dtype, omega, fl, uw, rho, u, steps, b=6, bulk_one=True, boxes=None):
     """max error of the CUDA path against the oracle over all sample boxes after `steps` steps
     (g must already have done them)"""
     npdt = np.float32 if dtype == "f32" else np.float64
@@ -74,7 +74,7 @@ def subbox_error(g, oracle, n, Q, model, dtype, omega, fl, uw, rho, u, steps, b=
     u3 = u.reshape(3, n, n, n)
     _, t, _, _ = oracle.lattice(Q)
     worst = 0.0
-    for (x0, y0, z0) in sample_boxes(n, b):
+    for (x0, y0, z0) in (boxes or sample_boxes(n, b)):
         lo = [max(0, v - steps) for v in (x0, y0, z0)]
         hi = [min(n, v + b + steps) for v in (x0, y0, z0)]
         sl = tuple(slice(a, c) for a, c in zip(lo, hi))
@@ -253,3 +253,112 @@ def test_target_256_bgk_sampled(Lbm, oracle, scheme):
         g.step(steps)
         err = subbox_error(g, oracle, n, 19, "BGK_W2", "f64", omega, fl, uw, rho, u, steps)
         assert err <= TOL64, (steps, err)
+
+
+# ------------------------------------------------------------------ the 100-step gate at full size
+def _report(name, **kv):
+    """append one line to gpurun_out/parity_report.jsonl (scratch; summarised under profiles/)"""
+    import json
+    import os
+    d = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    try:
+        os.makedirs(d, exist_ok=True)
+        with open(os.path.join(d, "parity_report.jsonl"), "a") as fh:
+            fh.write(json.dumps(dict(test=name, **kv)) + "\n")
+    except OSError:
+        pass
+
+
+_oracle_256 = {}
+
+
+def oracle_target_256(oracle, steps):
+    """every population of the 256^3 target (D3Q19 BGK-W2 fp64 cavity, Re = 1000, seeded init) after
+    `steps` oracle steps; computed once per session (about 17 M cells x 100 steps on the host cores)"""
+    if steps not in _oracle_256:
+        n = 256
+        fl, uw, rho, u, omega = cavity(n, 1000)
+        o = oracle.Oracle(n, n, n, Q=19, model="BGK_W2", omega=omega)
+        o.set_flags(fl, uw)
+        o.init_equilibrium(rho, u)
+        o.step(steps)
+        _oracle_256.clear()
+        _oracle_256[steps] = (o.get_populations(), o.kinetic_energy())
+        del o
+    return _oracle_256[steps]
+
+
+@pytest.mark.parametrize("scheme", ["2POP_SOA", "AA_SOA"])
+def test_target_256_bgk_every_population_100_steps(Lbm, oracle, scheme):
+    """north_star's gate on the target itself: max |f_gpu - f_oracle| <= 1e-12 over EVERY population of
+    EVERY fluid cell of the 256^3 cavity after 100 steps, in the launch configuration bench.py times
+    ("identical results"; readings R23, R24)."""
+    n, steps = 256, 100
+    fl, uw, rho, u, omega = cavity(n, 1000)
+    fo, eo = oracle_target_256(oracle, steps)
+    g = make_gpu(Lbm, n, 19, "BGK_W2", scheme, "f64", omega, fl, uw, rho, u)
+    g.step(steps)
+    fg = g.get_populations()
+    eg = g.kinetic_energy()
+    g.close()
+    assert np.isfinite(fg).all()
+    fluid = fl.reshape(-1) == 0
+    err = 0.0
+    for k in range(19):      # plane by plane: no 2.5 GB temporaries
+        err = max(err, float(np.abs(fg[k] - fo[k])[fluid].max()))
+        assert np.all(fg[k][~fluid] == 0.0)
+    _report("target_256_100_steps", scheme=scheme, max_abs=err, energy_gpu=eg, energy_oracle=eo)
+    assert err <= TOL64, err
+    assert abs(eg - eo) <= 1e-12 * max(1.0, abs(eo))
+
+
+@pytest.mark.parametrize("scheme", ["2POP_SOA", "AA_SOA"])
+@pytest.mark.parametrize("model", ["TRT", "REG"])
+def test_config3_fp32_500_steps_beyond_l2(Lbm, oracle, model, scheme):
+    """config 3's step count (500) in fp32 against the fp64 oracle on a lattice beyond L2 (112 x 96 x 130,
+    1.4 M cells, 106 MB per array: the strided-prefetch path of the fp32 kernels), every population;
+    the 100-step gate (<= 2e-5 relative, R20) and the 500-step error are reported separately (R24)."""
+    nx, ny, nz = 112, 96, 130
+    fl = inputs.cavity_flags(nx, ny, nz)
+    uw = (inputs.U_LID, 0.0, 0.0)
+    rho, u = inputs.seeded_init(nx, ny, nz, 0)
+    omega = inputs.omega_from_re(256, 1000)            # config 3's relaxation rate
+    rho32, u32 = rho.astype(np.float32), u.astype(np.float32)
+    g = Lbm(nx, ny, nz, lattice=19, collision=model, scheme=scheme, omega=omega, dtype="f32")
+    g.set_flags(fl, uw)
+    g.init_equilibrium(rho32, u32)
+    o = oracle.Oracle(nx, ny, nz, Q=19, model=model, omega=omega)
+    o.set_flags(fl, uw)
+    o.init_equilibrium(rho32.astype(np.float64), u32.astype(np.float64))   # the rounded inputs (R20)
+    _, t, _, _ = oracle.lattice(19)
+    fluid = fl.reshape(-1) == 0
+    errs = {}
+    done = 0
+    for target in (100, 500):
+        g.step(target - done)
+        o.step(target - done)
+        done = target
+        fg = g.get_populations().astype(np.float64)
+        fo = o.get_populations()
+        assert np.isfinite(fg).all()
+        d = np.abs(fg - fo)[:, fluid]
+        errs[target] = (float((d / np.maximum(np.abs(fo[:, fluid]), t[:, None])).max()), float(d.max()))
+    g.close()
+    _report("config3_fp32_500_steps", model=model, scheme=scheme, rel_100=errs[100][0], abs_100=errs[100][1],
+            rel_500=errs[500][0], abs_500=errs[500][1])
+    assert errs[100][0] <= TOL32, errs
+    assert errs[500][0] <= TOL32, errs
+
+
+@pytest.mark.parametrize("scheme,steps", [("2POP_SOA", 100), ("AA_SOA", 100), ("AA_SOA", 101)])
+def test_config3_256_sampled_100_steps(Lbm, oracle, scheme, steps):
+    """config 3 (TRT, fp64) at the 100-step gate on the full 256^3 lattice: sampled boxes whose domain of
+    dependence (100 cells each way) the oracle steps; the lid-corner box alone spans 106^3 cells."""
+    n = 256
+    fl, uw, rho, u, omega = cavity(n, 1000)
+    g = make_gpu(Lbm, n, 19, "TRT", scheme, "f64", omega, fl, uw, rho, u)
+    g.step(steps)
+    err = subbox_error(g, oracle, n, 19, "TRT", "f64", omega, fl, uw, rho, u, steps, boxes=[(1, 1, n - 7), (n // 2, n // 2, n // 2)])
+    g.close()
+    _report("config3_256_sampled_100", scheme=scheme, steps=steps, max_abs=err)
+    assert err <= TOL64, err
