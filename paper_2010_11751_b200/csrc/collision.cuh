@@ -22,7 +22,20 @@
 
 namespace lbm {
 
-enum Model { M_BGK_W2 = 0, M_BGK_NW4, M_TRT, M_RM, M_HM, M_CM, M_CHM, M_K, M_RR, M_REG };
+enum Model { M_BGK_W2 = 0, M_BGK_NW4, M_TRT, M_RM, M_HM, M_CM, M_CHM, M_K, M_RR, M_REG,
+             // the same five moment-space models compiled for "every moment of order >= 3 relaxed with
+             // exactly 1": their post-collision value is the equilibrium, so the
+             // pre-collision moments of those orders are never computed
+             M_EQHI_FIRST, M_RM_E = M_EQHI_FIRST, M_HM_E, M_CM_E, M_CHM_E, M_K_E, M_COUNT };
+
+__host__ __device__ constexpr bool model_eq_hi(int model) { return model >= M_EQHI_FIRST; }
+// the model a variant computes
+__host__ __device__ constexpr int model_base(int model) { return model >= M_EQHI_FIRST ? model - M_EQHI_FIRST + M_RM : model; }
+// the variant of a model with orders >= 3 equilibrated, or the model itself when it has none
+__host__ __device__ constexpr int model_eq_variant(int model)
+{
+    return (model >= M_RM && model <= M_K) ? model - M_RM + M_EQHI_FIRST : model;
+}
 
 template <class T>
 struct Rates {
@@ -217,7 +230,10 @@ __device__ __forceinline__ T eq_factor(T v)
 
 // Eq 11 on every moment of order >= 2, Eq 13-15 on the three diagonal second-order ones.
 // `scale` multiplies the per-unit-density equilibrium (rho for moments of f, 1 for cumulants).
-template <int Q, int BASIS, class T>
+// EQHI: the rates of every order >= 3 are exactly 1, so those moments are SET to their equilibrium
+// (PAPER.md:L340-342); nothing reads their pre-collision values any more and the compiler drops the
+// part of the forward transform that produced them (the code is fully unrolled, registers only).
+template <int Q, int BASIS, bool EQHI = false, class T>
 __device__ __forceinline__ void relax_moments(T (&m)[27], T scale, const T (&u)[3], const Rates<T>& rt)
 {
     using L = Lat<Q>;
@@ -232,8 +248,12 @@ __device__ __forceinline__ void relax_moments(T (&m)[27], T scale, const T (&u)[
             const T meq = (BASIS == B_CUMULANT)
                               ? T(0)
                               : scale * eq_factor<BASIS, p>(u[0]) * eq_factor<BASIS, q>(u[1]) * eq_factor<BASIS, r>(u[2]);
-            const T w = order == 2 ? rt.omega : order == 3 ? rt.omega3 : rt.omega_hi;
-            m[ic] = m[ic] - w * (m[ic] - meq);
+            if constexpr (EQHI && order >= 3) {
+                m[ic] = meq;
+            } else {
+                const T w = order == 2 ? rt.omega : order == 3 ? rt.omega3 : rt.omega_hi;
+                m[ic] = m[ic] - w * (m[ic] - meq);
+            }
         }
     });
     m[18] = m[18] - wp * n200 - wm * n020 - wm * n002;  // Eq 13
@@ -274,10 +294,12 @@ __device__ __forceinline__ void equilibrium_ext(T rho, const T (&u)[3], T (&E)[Q
 
 // ---------------------------------------------------------------- the operator
 // f (or g = f - t when SHIFT) in, post-collision value out, in place.
-template <int Q, int MODEL, bool SHIFT, class T>
+template <int Q, int MODEL_OR_VARIANT, bool SHIFT, class T>
 __device__ __forceinline__ void collide(T (&f)[Q], const Rates<T>& rt)
 {
     using L = Lat<Q>;
+    constexpr int MODEL = model_base(MODEL_OR_VARIANT);
+    constexpr bool EQHI = model_eq_hi(MODEL_OR_VARIANT);
     T rho, drho, u[3];
     moments_rho_u<Q, SHIFT>(f, rho, drho, u);
 
@@ -375,19 +397,19 @@ __device__ __forceinline__ void collide(T (&f)[Q], const Rates<T>& rt)
             r1.omega_bulk = rt.omega; r1.omega3 = rt.omega; r1.omega_hi = rt.omega;
             relax_moments<Q, B_RAW>(m, rho, u, r1);
         } else if constexpr (MODEL == M_RM) {
-            relax_moments<Q, B_RAW>(m, rho, u, rt);
+            relax_moments<Q, B_RAW, EQHI>(m, rho, u, rt);
         } else if constexpr (MODEL == M_HM) {
             basis_map<Q, TO_HERMITE>(m, u);
-            relax_moments<Q, B_HERMITE>(m, rho, u, rt);
+            relax_moments<Q, B_HERMITE, EQHI>(m, rho, u, rt);
             basis_map<Q, FROM_HERMITE>(m, u);
         } else if constexpr (MODEL == M_CM) {
             basis_map<Q, TO_CENTRAL>(m, u);
-            relax_moments<Q, B_CENTRAL>(m, rho, u, rt);
+            relax_moments<Q, B_CENTRAL, EQHI>(m, rho, u, rt);
             basis_map<Q, FROM_CENTRAL>(m, u);
         } else if constexpr (MODEL == M_CHM) {
             basis_map<Q, TO_CENTRAL>(m, u);
             basis_map<Q, TO_HERMITE>(m, u);
-            relax_moments<Q, B_CENTRAL_HERMITE>(m, rho, u, rt);
+            relax_moments<Q, B_CENTRAL_HERMITE, EQHI>(m, rho, u, rt);
             basis_map<Q, FROM_HERMITE>(m, u);
             basis_map<Q, FROM_CENTRAL>(m, u);
         } else if constexpr (MODEL == M_K) {
@@ -398,7 +420,7 @@ __device__ __forceinline__ void collide(T (&f)[Q], const Rates<T>& rt)
                 if constexpr (L::has_moment(ic / 9, (ic / 3) % 3, ic % 3)) m[ic] *= inv;
             });
             cumulants_fwd<Q>(m);
-            relax_moments<Q, B_CUMULANT>(m, T(1), u, rt);
+            relax_moments<Q, B_CUMULANT, EQHI>(m, T(1), u, rt);
             cumulants_bwd<Q>(m);
             static_for<27>([&](auto ic) {
                 if constexpr (L::has_moment(ic / 9, (ic / 3) % 3, ic % 3)) m[ic] *= rho;

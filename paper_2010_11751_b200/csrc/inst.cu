@@ -1,10 +1,10 @@
 // inst.cu -- step kernels of ONE (lattice, collision model) pair; compiled once per pair with
-//   -DLBM_INST_Q=<19|27> -DLBM_INST_MODEL=<0..9>
+//   -DLBM_INST_Q=<19|27> -DLBM_INST_MODEL=<0..14>  (collision.cuh: enum Model)
 // (see paper_2010_11751_b200/build.py).  fp64 and fp32 (shifted storage, R20).
 #include "dispatch.cuh"
 
 #ifndef LBM_INST_Q
-#error "compile with -DLBM_INST_Q=19|27 -DLBM_INST_MODEL=0..9"
+#error "compile with -DLBM_INST_Q=19|27 -DLBM_INST_MODEL=0..14"
 #endif
 
 namespace lbm {

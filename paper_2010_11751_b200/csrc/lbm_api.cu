@@ -1,6 +1,6 @@
 // lbm_api.cu -- the C ABI of include/lbm.h: context, state machine of the schemes, argument
 // checks and kernel launches.  No arithmetic of the method lives here; every step of the path
-// runs in the kernels of kernels.cuh / fast19.cuh.
+// runs in the kernels of kernels.cuh / collision.cuh / aux.cu.
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -172,6 +172,18 @@ cudaError_t step_model(const lbm_ctx* c, int kind, const StepArgs<T>& a)
     case LBM_TRT: return launch_step<T, Q, M_TRT>(kind, soa, b, st, a, s);
     case LBM_REG: return launch_step<T, Q, M_REG>(kind, soa, b, st, a, s);
     default: break;
+    }
+    // every moment of order >= 3 relaxed with exactly 1: the variant that never computes their
+    // pre-collision values (collision.cuh).  Same result up to round-off.
+    if (c->omega3 == 1.0 && c->omega_hi == 1.0) {
+        switch (c->model) {
+        case LBM_RM: return launch_step<T, Q, M_RM_E>(kind, soa, b, st, a, s);
+        case LBM_HM: return launch_step<T, Q, M_HM_E>(kind, soa, b, st, a, s);
+        case LBM_CM: return launch_step<T, Q, M_CM_E>(kind, soa, b, st, a, s);
+        case LBM_CHM: return launch_step<T, Q, M_CHM_E>(kind, soa, b, st, a, s);
+        case LBM_K: return launch_step<T, Q, M_K_E>(kind, soa, b, st, a, s);
+        default: break;
+        }
     }
     {
         switch (c->model) {
