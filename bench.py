@@ -351,15 +351,15 @@ def run_gpu_slab(args):
     dev = torch.device("cuda", local_rank)
     from paper_2010_11751_b200 import slab
     n, Q, model, scheme, dtype, re = WORKLOADS[args.workload]
-    if scheme != "2POP_SOA":
-        raise SystemExit("--decomp slab needs a two-population SoA workload (target2pop, 1)")
+    if not scheme.endswith("SOA"):
+        raise SystemExit("--decomp slab needs an SoA workload")
     K, W = args.steps, max(args.warmup, 3)
     NX = world * n
     omega = inputs.omega_from_re(n, re)
     x0, x1 = slab.slab_range(NX, rank, world)
     fl, rho, u = slab.cavity_slab(NX, n, n, x0, x1, seed=0)
     g = slab.SlabLbm(NX, n, n, flags_local=fl, u_wall=(inputs.U_LID, 0.0, 0.0), dist=dist, rank=rank, world=world,
-                     lattice=Q, collision=model, omega=omega, dtype=dtype)
+                     lattice=Q, collision=model, omega=omega, dtype=dtype, scheme=scheme, transport=args.transport)
     nfluid = g.num_fluid
 
     def barrier():
@@ -407,8 +407,10 @@ def run_gpu_slab(args):
     achieved = nfluid * bpu / (step_ms * 1e-3) / 1e9
     cfg = workload_config(args.workload, world)
     cfg["workload"] = "%s, as ONE %d x %d x %d cavity cut into %d x-slabs" % (cfg["workload"], NX, n, n, world)
-    cfg["parallelism"] = "slab x%d along x, one-cell halo: %d of %d planes per face per step over torch.distributed p2p" % (
-        world, 5 if Q == 19 else 9, Q)
+    cfg["parallelism"] = "slab x%d along x, one-cell halo: %d of %d planes per face per step, transport %s" % (
+        world, 5 if Q == 19 else 9, Q,
+        "peer stores from the pack kernel into the neighbour's receive buffer (lbm_slab_step)" if g.transport == "peer"
+        else "torch.distributed p2p")
     nloc = (x1 - x0 + 2) * n * n
     line = {
         "metric": METRIC, "value": units_g / (ms_total_g * 1e-3) / 1e6, "unit": UNIT, "n_gpus": world, "steps": K,
@@ -438,6 +440,8 @@ def main():
                     help="any other case N,Q,MODEL,SCHEME,DTYPE[,RE], e.g. 256,19,BGK_W2,2POP_AOS,f64 (overrides --workload)")
     ap.add_argument("--variant", default=None, help="step-kernel variant (binding.VARIANTS), default = library's choice")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--transport", default=None, choices=["peer", "p2p"],
+                    help="--decomp slab: library driver over peer memory / torch.distributed send-recv (default: peer for one rank, p2p otherwise)")
     ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
                     help="replicas (default): N independent lattices; slab: one lattice cut along x with a halo exchange")
     args = ap.parse_args()

@@ -123,33 +123,67 @@ int lbm_set_variant(lbm_t* ctx, int variant);
  * default 128).  Results do not depend on it. */
 int lbm_set_block(lbm_t* ctx, int threads);
 
-/* Halo exchange of a slab decomposition along x (the slowest axis: an x-layer is ny*nz contiguous
- * cells of every SoA plane).  The paper's scheme is single-device; cells are
- * coupled only through the one-cell stencil of Eq 2, so a rank owns the layers
- * x = 1 .. nx-2 of its context and flags x = 0 and x = nx-1 LBM_GHOST (or WALL/MOVING where the
- * neighbouring rank's layer is solid).  After every lbm_step(1):
- *   lbm_halo_pack(face, buf)    buf <- post-collision populations of the owned layer next to the
- *                               face that leave through it: face 0 (low x): cx = -1 of layer 1;
- *                               face 1 (high x): cx = +1 of layer nx-2;
- *   (send buf to that neighbour; receive its buffer of the opposite face)
- *   lbm_halo_unpack(face, buf)  ghost layer of the face <- buf (face 0: cx = +1 into layer 0;
- *                               face 1: cx = -1 into layer nx-1).
- * buf is DEVICE memory of lbm_halo_count() elements of the context dtype, layout [dir][ny*nz] with
- * directions in increasing k; asynchronous on the stream.  Two-population SoA scheme only
- * (LBM_E_ARG otherwise); raw stored values, so both ranks must use the same dtype. */
-/* One time step in two parts, so that the halo exchange overlaps the bulk of the update:
- *   lbm_step_begin   updates the outermost owned layers x = 1 and x = nx-2 only;
- *   lbm_halo_pack    (both faces) then reads the new values of those layers; start the exchange;
- *   lbm_step_end     updates the layers 2 .. nx-3 and completes the step;
- *   lbm_halo_unpack  (both faces) once the neighbours' buffers have arrived.
- * Layers 0 and nx-1 are not updated by this pair: they must be GHOST or solid.  The result is
- * bit for bit that of lbm_step(1).  Between begin and end only lbm_halo_pack is allowed
- * (LBM_E_STATE otherwise).  Two-population SoA scheme only. */
+/* Slab decomposition along x (the slowest axis: an x-layer is ny*nz contiguous cells of every SoA
+ * plane).  The paper's scheme is single-device; cells are coupled only through the
+ * one-cell stencil of Eq 2, so a rank owns the layers x = 1 .. nx-2 of its context
+ * and flags x = 0 and x = nx-1 LBM_GHOST (or WALL/MOVING where the neighbouring rank's layer is
+ * solid).  SoA schemes only (two-population in its pull form, swap, AA); LBM_E_ARG otherwise, and
+ * lbm_set_flags refuses LBM_GHOST cells there.
+ *
+ * One time step in parts, so that the halo travels while the bulk of the slab is updated:
+ *   lbm_step_begin    the step's kernel on the outermost owned layers x = 1 and x = nx-2 only
+ *                     (swap: pass 1).  Layers 0 and nx-1 are never updated: LBM_E_STATE if they
+ *                     hold a FLUID cell;
+ *   lbm_halo_pack     (both faces) buf <- what leaves through the face; start the transfer;
+ *   lbm_step_end      the same kernel on the layers 2 .. nx-3;
+ *   lbm_halo_unpack   (both faces) once the neighbours' buffers have arrived;
+ *   lbm_step_finish   completes the step (swap: pass 2, which needs the halo).
+ * Between begin and finish no other call on the context is allowed (LBM_E_STATE).  The result is
+ * bit for bit that of the undivided lattice.  What a message holds depends on the scheme (Table 1,
+ * PAPER.md:L147-159; 5 of 19 or 9 of 27 directions per face, those with c_x pointing out of it, in
+ * increasing k, layout [dir][ny*nz], raw stored values of the context dtype):
+ *   two-population   post-collision f_out_k of the outermost owned layer (slot k); unpack writes
+ *                    the ghost layer, from which the next step pulls;
+ *   AA, even step    the same values, which this step keeps in slot kbar; unpack writes the ghost
+ *                    layer ("AA exchanges on odd steps only": the odd step pulls them from there);
+ *   AA, odd step     the odd step pushes into slot k of x + c_k, i.e. into the ghost layer: pack
+ *                    reads the ghost layer, unpack merges into the neighbour's outermost owned
+ *                    layer, skipping cells whose upstream cell is solid (they bounced back);
+ *   swap             after pass 1 (as AA even); through the low face the ghost layer is written,
+ *                    through the high face the half of the pass-2 exchange that the (absent) thread
+ *                    of the ghost cell would have done is applied on arrival.
+ * A context with GHOST cells stepped by plain lbm_step(1) (two-population, AA) needs pack / unpack
+ * after every step; lbm_step(n > 1) and the swap scheme return LBM_E_STATE there.
+ * buf is DEVICE memory of lbm_halo_count() elements; every call is asynchronous on the stream. */
 int lbm_step_begin(lbm_t* ctx);
 int lbm_step_end(lbm_t* ctx);
+int lbm_step_finish(lbm_t* ctx);
 long long lbm_halo_count(const lbm_t* ctx);
 int lbm_halo_pack(lbm_t* ctx, int face, void* buf_dev);
 int lbm_halo_unpack(lbm_t* ctx, int face, const void* buf_dev);
+
+/* The same step driven inside the library, the halo stored by the pack kernel straight into the
+ * neighbouring slab's receive buffer (peer memory: NVLink between GPUs) and a sequence number
+ * published behind it; the neighbour's unpack kernel waits for that number (bounded).  No host
+ * code runs between the parts and nothing goes through a communication library.
+ *   lbm_slab_link(ctx, face, peer)   the slab beyond `face` is context `peer` of this process (any
+ *                                    device with peer access; peer == ctx closes a periodic ring of
+ *                                    one slab; NULL = nothing beyond: that face is never exchanged);
+ *   lbm_slab_export / lbm_slab_import   the same across processes through a 64-byte CUDA IPC
+ *                                    handle of the receive block (export mine, import the
+ *                                    neighbour's for `face`); same ny, nz, lattice, scheme, dtype;
+ *   lbm_slab_post      lbm_step_begin, both peer stores, lbm_step_end;
+ *   lbm_slab_complete  both merges, lbm_step_finish;
+ *   lbm_slab_step(n)   n times post + complete (every slab on its own device and stream).  Several
+ *                      slabs on ONE stream must alternate instead: post on all, then complete on all;
+ *   lbm_slab_status    LBM_E_STATE if some message never arrived (synchronises). */
+int lbm_slab_link(lbm_t* ctx, int face, lbm_t* peer);
+int lbm_slab_export(lbm_t* ctx, void* handle64);
+int lbm_slab_import(lbm_t* ctx, int face, const void* handle64);
+int lbm_slab_post(lbm_t* ctx);
+int lbm_slab_complete(lbm_t* ctx);
+int lbm_slab_step(lbm_t* ctx, int n);
+int lbm_slab_status(lbm_t* ctx);
 
 /* CUDA-graph replay of lbm_step.  A step of a small lattice lasts a few microseconds and is bound
  * by launch latency (the paper's "one synchronisation per step"), and up to ~128^3

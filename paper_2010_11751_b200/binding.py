@@ -19,7 +19,7 @@ MODELS = {"BGK_W2": 0, "BGK_NW4": 1, "TRT": 2, "RM": 3, "HM": 4, "CM": 5, "CHM":
 SCHEMES = {"2POP_SOA": 0, "2POP_AOS": 1, "SWAP_SOA": 2, "SWAP_AOS": 3, "AA_SOA": 4, "AA_AOS": 5}
 DTYPES = {"f32": 0, "f64": 1}
 NP_DTYPES = {"f32": np.float32, "f64": np.float64}
-VARIANTS = {"default": 0, "generic_push": 1, "generic_pull": 2, "aos_plain": 3}
+VARIANTS = {"default": 0, "generic_push": 1, "generic_pull": 2, "aos_plain": 3, "tma": 4, "no_tma": 5}
 FLUID, WALL, MOVING, GHOST = 0, 1, 2, 3
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
@@ -27,7 +27,9 @@ SYMBOLS = [
     "lbm_set_hooks", "lbm_create", "lbm_destroy", "lbm_set_flags", "lbm_set_relaxation", "lbm_set_trt_magic",
     "lbm_init_equilibrium", "lbm_init_equilibrium_device", "lbm_step", "lbm_macroscopic", "lbm_macroscopic_device", "lbm_kinetic_energy", "lbm_kinetic_energy_device", "lbm_get_populations", "lbm_get_populations_at",
     "lbm_set_populations", "lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches",
-    "lbm_sync", "lbm_set_variant", "lbm_set_block", "lbm_set_graph", "lbm_graph_replays", "lbm_halo_count", "lbm_halo_pack", "lbm_halo_unpack", "lbm_step_begin", "lbm_step_end", "lbm_last_error", "lbm_version",
+    "lbm_sync", "lbm_set_variant", "lbm_set_block", "lbm_set_graph", "lbm_graph_replays", "lbm_halo_count", "lbm_halo_pack", "lbm_halo_unpack", "lbm_step_begin", "lbm_step_end", "lbm_step_finish",
+    "lbm_slab_link", "lbm_slab_export", "lbm_slab_import", "lbm_slab_post", "lbm_slab_complete", "lbm_slab_step", "lbm_slab_status",
+    "lbm_last_error", "lbm_version",
 ]
 GRAPH_MODES = {"auto": 0, "off": 1, "on": 2}
 
@@ -73,6 +75,14 @@ def load_library(path=LIB_PATH):
     L.lbm_set_graph.argtypes = [vp, i]
     L.lbm_step_begin.argtypes = [vp]
     L.lbm_step_end.argtypes = [vp]
+    L.lbm_step_finish.argtypes = [vp]
+    L.lbm_slab_link.argtypes = [vp, i, vp]
+    L.lbm_slab_export.argtypes = [vp, vp]
+    L.lbm_slab_import.argtypes = [vp, i, vp]
+    L.lbm_slab_post.argtypes = [vp]
+    L.lbm_slab_complete.argtypes = [vp]
+    L.lbm_slab_step.argtypes = [vp, i]
+    L.lbm_slab_status.argtypes = [vp]
     L.lbm_halo_count.restype = C.c_longlong
     L.lbm_halo_count.argtypes = [vp]
     L.lbm_halo_pack.argtypes = [vp, i, vp]
@@ -249,6 +259,34 @@ class Lbm:
 
     def step_end(self):
         self._ck(self._L.lbm_step_end(self._h))
+
+    def step_finish(self):
+        self._ck(self._L.lbm_step_finish(self._h))
+
+    def slab_link(self, face, peer):
+        """the slab beyond `face` is the context `peer` of this process (None = nothing beyond)"""
+        self._ck(self._L.lbm_slab_link(self._h, int(face), peer._h if peer is not None else None))
+
+    def slab_export(self):
+        """64-byte CUDA IPC handle of this context's halo receive block"""
+        h = C.create_string_buffer(64)
+        self._ck(self._L.lbm_slab_export(self._h, h))
+        return h.raw
+
+    def slab_import(self, face, handle):
+        self._ck(self._L.lbm_slab_import(self._h, int(face), C.create_string_buffer(bytes(handle), 64)))
+
+    def slab_post(self):
+        self._ck(self._L.lbm_slab_post(self._h))
+
+    def slab_complete(self):
+        self._ck(self._L.lbm_slab_complete(self._h))
+
+    def slab_step(self, n=1):
+        self._ck(self._L.lbm_slab_step(self._h, int(n)))
+
+    def slab_status(self):
+        self._ck(self._L.lbm_slab_status(self._h))
 
     @property
     def halo_count(self):

@@ -9,14 +9,9 @@ namespace lbm {
 // mask is non-zero: a link of the lattice ends on a non-fluid cell, or the cell lies on a face of
 // the box (periodic seam).
 template <int Q>
-__global__ void classify_kernel(const uint8_t* __restrict__ flags, uint8_t* __restrict__ code,
-                                unsigned long long* __restrict__ mask, Geo g)
+__device__ __forceinline__ unsigned long long link_mask(const uint8_t* __restrict__ flags, const Geo& g, int i)
 {
     using L = Lat<Q>;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= g.n) return;
-    const uint8_t fl = flags[i];
-    if (fl != 0) { code[i] = fl == 2 ? CODE_MOVING : fl == 3 ? CODE_GHOST : CODE_WALL; mask[i] = 0ull; return; }
     const int z = i % g.nz, y = (i / g.nz) % g.ny, x = i / (g.nz * g.ny);
     unsigned long long m = 0ull;
     if (x == 0) m |= 1ull << (MASK_FACE_SHIFT + 0);
@@ -34,8 +29,58 @@ __global__ void classify_kernel(const uint8_t* __restrict__ flags, uint8_t* __re
             if (nf == 2) m |= 1ull << (MASK_MOVING_SHIFT + link_of<Q>(k));
         }
     });
-    code[i] = m ? CODE_EDGE : CODE_BULK;
-    mask[i] = m;
+    return m;
+}
+
+// pass 1: the code byte of every cell and, per aligned group of 32 cells (one warp), the bit set of
+// its edge cells (grp.y) and their number (grp.x, turned into an exclusive prefix sum by pass 2)
+template <int Q>
+__global__ void __launch_bounds__(256) classify_kernel(const uint8_t* __restrict__ flags, uint8_t* __restrict__ code,
+                                                        uint2* __restrict__ grp, Geo g)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool edge = false;
+    if (i < g.n) {
+        const uint8_t fl = flags[i];
+        uint8_t c;
+        if (fl != 0) c = fl == 2 ? CODE_MOVING : fl == 3 ? CODE_GHOST : CODE_WALL;
+        else { edge = link_mask<Q>(flags, g, i) != 0ull; c = edge ? CODE_EDGE : CODE_BULK; }
+        code[i] = c;
+    }
+    const unsigned bits = __ballot_sync(0xffffffffu, edge);
+    if ((threadIdx.x & 31) == 0 && i < g.n) grp[i >> 5] = make_uint2((unsigned)__popc(bits), bits);
+}
+
+// pass 2: exclusive prefix sum of grp[].x over the ngrp groups, one block; total[0] = number of edge cells
+__global__ void __launch_bounds__(1024) classify_scan_kernel(uint2* __restrict__ grp, int ngrp, unsigned* __restrict__ total)
+{
+    __shared__ unsigned part[1024];
+    const int per = (ngrp + 1023) / 1024;
+    const int lo = min(ngrp, (int)threadIdx.x * per), hi = min(ngrp, lo + per);
+    unsigned s = 0;
+    for (int j = lo; j < hi; ++j) s += grp[j].x;
+    part[threadIdx.x] = s;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {   // inclusive scan of the per-thread sums
+        const unsigned v = threadIdx.x >= (unsigned)o ? part[threadIdx.x - o] : 0u;
+        __syncthreads();
+        part[threadIdx.x] += v;
+        __syncthreads();
+    }
+    unsigned run = part[threadIdx.x] - s;
+    for (int j = lo; j < hi; ++j) { const unsigned cnt = grp[j].x; grp[j].x = run; run += cnt; }
+    if (threadIdx.x == 1023) total[0] = part[1023];
+}
+
+// pass 3: the masks of the edge cells, in cell order
+template <int Q>
+__global__ void __launch_bounds__(256) classify_mask_kernel(const uint8_t* __restrict__ flags, const uint8_t* __restrict__ code,
+                                                             const uint2* __restrict__ grp, unsigned long long* __restrict__ mask, Geo g)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.n || code[i] != CODE_EDGE) return;
+    const uint2 gg = grp[i >> 5];
+    mask[gg.x + __popc(gg.y & ((1u << (i & 31)) - 1u))] = link_mask<Q>(flags, g, i);
 }
 
 // energy stages 2 and 3: block b sums the contiguous segment [b*seg, min(n, (b+1)*seg)) of `in` in a
@@ -63,7 +108,7 @@ template <class T, int Q, bool SOA>
 __global__ void __launch_bounds__(256) stream_only_kernel(const StepArgs<T> a)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
+    const CellState cs = cell_state(a, i, a.g.n);
     if (!cs.active) return;
     T f[Q];
     load_cell<T, Q, SOA, LD_PULL>(a, i, cs.masked, cs.mask, f);
@@ -72,10 +117,19 @@ __global__ void __launch_bounds__(256) stream_only_kernel(const StepArgs<T> a)
 
 static inline int blocks_for(int n, int block) { return (n + block - 1) / block; }
 
-cudaError_t aux_classify(int Q, const uint8_t* flags, uint8_t* code, unsigned long long* mask, const Geo& g, cudaStream_t s)
+cudaError_t aux_classify_codes(int Q, const uint8_t* flags, uint8_t* code, uint2* grp, unsigned* total, const Geo& g, cudaStream_t s)
 {
-    if (Q == 19) classify_kernel<19><<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, mask, g);
-    else if (Q == 27) classify_kernel<27><<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, mask, g);
+    if (Q == 19) classify_kernel<19><<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, grp, g);
+    else if (Q == 27) classify_kernel<27><<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, grp, g);
+    else return cudaErrorInvalidValue;
+    classify_scan_kernel<<<1, 1024, 0, s>>>(grp, (g.n + 31) / 32, total);
+    return cudaGetLastError();
+}
+cudaError_t aux_classify_masks(int Q, const uint8_t* flags, const uint8_t* code, const uint2* grp, unsigned long long* mask,
+                               const Geo& g, cudaStream_t s)
+{
+    if (Q == 19) classify_mask_kernel<19><<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, grp, mask, g);
+    else if (Q == 27) classify_mask_kernel<27><<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, grp, mask, g);
     else return cudaErrorInvalidValue;
     return cudaGetLastError();
 }
@@ -199,11 +253,11 @@ cudaError_t aux_stream_only(int Q, bool soa, const StepArgs<T>& a, cudaStream_t 
 }
 
 template <class T>
-cudaError_t aux_halo(bool pack, T* pop, long long stride, const HaloArgs& p, T* buf, cudaStream_t s)
+cudaError_t aux_halo(bool pack, T* pop, const uint8_t* code, long long stride, const HaloArgs& p, T* buf, cudaStream_t s)
 {
     const dim3 grid((p.cells + 255) / 256, p.ndir);
-    if (pack) halo_kernel<T, true><<<grid, 256, 0, s>>>(pop, stride, p, buf);
-    else halo_kernel<T, false><<<grid, 256, 0, s>>>(pop, stride, p, buf);
+    if (pack) halo_kernel<T, true><<<grid, 256, 0, s>>>(pop, code, stride, p, buf);
+    else halo_kernel<T, false><<<grid, 256, 0, s>>>(pop, code, stride, p, buf);
     return cudaGetLastError();
 }
 
@@ -216,7 +270,7 @@ cudaError_t aux_halo(bool pack, T* pop, long long stride, const HaloArgs& p, T* 
                                               const int*, int, cudaStream_t);                                                           \
     template cudaError_t aux_insert_plane<T>(int, bool, T*, const uint8_t*, const Geo&, int, double, const T*,          \
                                              cudaStream_t);                                                             \
-    template cudaError_t aux_halo<T>(bool, T*, long long, const HaloArgs&, T*, cudaStream_t);                           \
+    template cudaError_t aux_halo<T>(bool, T*, const uint8_t*, long long, const HaloArgs&, T*, cudaStream_t);                           \
     template cudaError_t aux_swap_stream<T>(int, bool, const StepArgs<T>&, cudaStream_t);                               \
     template cudaError_t aux_stream_only<T>(int, bool, const StepArgs<T>&, cudaStream_t);
 LBM_AUX_INST(float)

@@ -22,6 +22,8 @@ enum Variant {
     V_GENERIC_PUSH,  // generic one-thread-per-cell kernels, 2-pop as collide-then-push
     V_GENERIC_PULL,  // generic kernels, 2-pop as pull-then-collide with lazily streamed storage
     V_AOS_PLAIN,     // AoS without the shared-memory tile (every access a per-thread gather / scatter)
+    V_TMA,           // SoA: loads staged through shared memory by TMA bulk copies (tma_step.cuh)
+    V_NO_TMA,        // SoA: never that kernel (one cell per thread, loads into registers, L2 prefetch)
     V_COUNT
 };
 
@@ -30,7 +32,11 @@ template <class T, int Q, int MODEL>
 cudaError_t launch_step(int kind, bool soa, int block, bool staged, const StepArgs<T>& a, cudaStream_t s);
 
 // defined in aux.cu
-cudaError_t aux_classify(int Q, const uint8_t* flags, uint8_t* code, unsigned long long* mask, const Geo& g, cudaStream_t s);
+// flags -> code bytes + per-group edge bits and ordinals (+ the number of edge cells in total[0]); then the
+// compact mask array, which the caller allocates from that number
+cudaError_t aux_classify_codes(int Q, const uint8_t* flags, uint8_t* code, uint2* grp, unsigned* total, const Geo& g, cudaStream_t s);
+cudaError_t aux_classify_masks(int Q, const uint8_t* flags, const uint8_t* code, const uint2* grp, unsigned long long* mask,
+                               const Geo& g, cudaStream_t s);
 template <class T>
 cudaError_t aux_init_equilibrium(int Q, bool ext, bool soa, T* pop, const uint8_t* code, const Geo& g, const T* rho,
                                  const T* u, cudaStream_t s);
@@ -49,7 +55,7 @@ cudaError_t aux_insert_plane(int Q, bool soa, T* pop, const uint8_t* code, const
 template <class T>
 cudaError_t aux_swap_stream(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s);
 template <class T>
-cudaError_t aux_halo(bool pack, T* pop, long long stride, const HaloArgs& p, T* buf, cudaStream_t s);
+cudaError_t aux_halo(bool pack, T* pop, const uint8_t* code, long long stride, const HaloArgs& p, T* buf, cudaStream_t s);
 // stream only (LD_PULL -> ST_LOCAL without collision): turns post-collision storage into canonical
 template <class T>
 cudaError_t aux_stream_only(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s);

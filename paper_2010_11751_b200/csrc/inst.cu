@@ -2,6 +2,7 @@
 //   -DLBM_INST_Q=<19|27> -DLBM_INST_MODEL=<0..14>  (collision.cuh: enum Model)
 // (see paper_2010_11751_b200/build.py).  fp64 and fp32 (shifted storage, R20).
 #include "dispatch.cuh"
+#include "tma_step.cuh"
 
 #ifndef LBM_INST_Q
 #error "compile with -DLBM_INST_Q=19|27 -DLBM_INST_MODEL=0..14"
@@ -17,6 +18,38 @@ static cudaError_t launch_one(int block, bool staged, const StepArgs<T>& a, cuda
             const int b = block > 128 ? 128 : block;
             step_kernel_aos<T, Q, MODEL, LOAD, STORE><<<(a.g.n + b - 1) / b, b, (size_t)b * Q * sizeof(T), s>>>(a);
             return cudaGetLastError();
+        }
+    }
+    // SoA, whole lattice: loads staged through shared memory by the TMA unit (tma_step.cuh)
+    if constexpr (SOA && ((LOAD == LD_PULL && STORE == ST_LOCAL) || (LOAD == LD_LOCAL && STORE == ST_SWAPPED) ||
+                          (LOAD == LD_AAPULL && STORE == ST_PUSH))) {
+        if (a.tma && a.first == 0 && a.end == a.g.n) {
+            constexpr int B = tma_tile<T, Q>(), S = tma_stages<T, Q>();
+            constexpr size_t smem = tma_smem_bytes<T, Q, B, S>();
+            auto kernel = step_kernel_tma<T, Q, MODEL, LOAD, STORE>;
+            static int per_sm = 0, sms = 0;   // per instantiation
+            if (!per_sm) {
+                cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                if (e != cudaSuccess) return e;
+                int dev = 0;
+                cudaGetDevice(&dev);
+                cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+                e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, B, smem);
+                if (e != cudaSuccess || per_sm < 1) { per_sm = 0; return e != cudaSuccess ? e : cudaErrorLaunchOutOfResources; }
+            }
+            const int ntiles = (a.g.n + B - 1) / B;
+            const int grid = ntiles < per_sm * sms ? ntiles : per_sm * sms;
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)grid);
+            cfg.blockDim = dim3((unsigned)B);
+            cfg.dynamicSmemBytes = smem;
+            cfg.stream = s;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+            attr[0].val.programmaticStreamSerializationAllowed = 1;
+            cfg.attrs = attr;
+            cfg.numAttrs = a.pdl ? 1 : 0;
+            return cudaLaunchKernelEx(&cfg, kernel, a);
         }
     }
     const int b = block > max_threads<T, Q>() ? max_threads<T, Q>() : block;

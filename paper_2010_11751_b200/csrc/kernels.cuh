@@ -17,6 +17,11 @@
 //   bits 26..51  link l: that neighbour is a MOVING wall
 //   bits 52..57  the cell lies on the face x=0, x=nx-1, y=0, y=ny-1, z=0, z=nz-1 (periodic seam)
 //
+// The masks are stored compactly, one per EDGE cell in cell order (a 512^3 cavity has 1.6 M of them,
+// not 134 M): `grp[i >> 5]` holds, per aligned group of 32 cells, the ordinal of the group's first
+// edge cell (x) and the bit set of its edge cells (y), so that the mask of edge cell i is
+// mask[grp.x + popc(grp.y & lanes below i)].  Side arrays: 1 B (code) + 0.25 B (grp) per cell.
+//
 // A warp in which no lane has a mask runs the pure path (fixed offsets, no tests); a warp with at
 // least one masked lane runs the masked path for all its lanes (selects on mask bits, no
 // divergence, no integer division).  Both give the same values for bulk cells.
@@ -45,12 +50,14 @@ struct StepArgs {
     const T* src;
     T* dst;
     const uint8_t* code;
-    const unsigned long long* mask;
+    const uint2* grp;                  // per 32 cells: ordinal of the first edge cell, bit set of edge cells
+    const unsigned long long* mask;    // link masks of the edge cells, in cell order
     Geo g;
     int first, end;   // the step kernel updates the cells [first, end): the whole box, or some x-layers (slab overlap)
     int pdl;          // host side: launch with programmatic stream serialisation (see step_kernel)
     int pf;           // L2 prefetch distance in cells (0 = off), see step_kernel
     int pf_strided;   // one warp in 128/sizeof(T) prefetches, each lane a different line
+    int tma;          // host side: run step_kernel_tma (tma_step.cuh) when the launch allows it
     Rates<T> rt;
     T wterm[27];  // w_k
     // offsets filled on the host per launch (make_args) so that the kernels add one uniform
@@ -194,18 +201,24 @@ struct CellState {
     bool partial;   // inactive lane of a warp that has active lanes
     unsigned long long mask;
 };
-__device__ __forceinline__ CellState cell_state(const uint8_t* __restrict__ code,
-                                                const unsigned long long* __restrict__ mask, long long i, int n)
+__device__ __forceinline__ unsigned long long edge_mask(const uint2* __restrict__ grp,
+                                                        const unsigned long long* __restrict__ mask, long long i)
+{
+    const uint2 g = grp[i >> 5];
+    return mask[g.x + __popc(g.y & ((1u << (i & 31)) - 1u))];
+}
+template <class ARGS>
+__device__ __forceinline__ CellState cell_state(const ARGS& a, long long i, int n)
 {
     CellState s;
     uint8_t c = CODE_WALL;
-    if (i < n) c = code[i];
+    if (i < n) c = a.code[i];
     s.active = !(c & 3);
     const bool edge = c == CODE_EDGE;
     s.masked = __any_sync(0xffffffffu, edge);
     const bool any_active = __any_sync(0xffffffffu, s.active);
     s.partial = any_active && !s.active && i < n;
-    s.mask = edge ? mask[i] : 0ull;
+    s.mask = edge ? edge_mask(a.grp, a.mask, i) : 0ull;
     return s;
 }
 
@@ -254,7 +267,7 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
     // the launch attribute both instructions do nothing.
     asm volatile("griddepcontrol.launch_dependents;");
     const int i = a.first + blockIdx.x * blockDim.x + threadIdx.x;
-    const CellState cs = cell_state(a.code, a.mask, i, a.end);
+    const CellState cs = cell_state(a, i, a.end);
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (!cs.active) {  // solid cells hold no populations
         // ... but when the other array is written (two-population), a warp that straddles a wall
@@ -283,8 +296,9 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
         // x-layer + one row + one cell beyond the target cell, so stay that far from both ends
         const long long margin = (long long)a.g.ny * a.g.nz + a.g.nz + 1;
         if (!a.pf_strided) {
-            if (i + a.pf >= margin && i + a.pf + margin < a.g.n && i + a.pf < a.end) {
-                const char* q = reinterpret_cast<const char*>(a.src + (long long)(i + a.pf) * (SOA ? 1 : Q));
+            const long long t = (long long)i + a.pf;   // 64-bit: N may be close to 2^31
+            if (t >= margin && t + margin < a.g.n && t < a.end) {
+                const char* q = reinterpret_cast<const char*>(a.src + t * (SOA ? 1 : Q));
                 static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(q + a.ldo[kc])); });
             }
         } else if constexpr (SOA) {
@@ -323,7 +337,7 @@ __global__ void __launch_bounds__(128) step_kernel_aos(const StepArgs<T> a)
     const long long base = (long long)blockIdx.x * blockDim.x;   // first cell of the block
     const int i = (int)base + threadIdx.x;
     const int nb = min((long long)blockDim.x, (long long)a.g.n - base) * Q;   // elements of the block's run
-    const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
+    const CellState cs = cell_state(a, i, a.g.n);
     T* rec = tile + threadIdx.x * Q;
     T f[Q];
     if constexpr (LOAD == LD_LOCAL) {
@@ -443,7 +457,7 @@ swap_stream_kernel(const StepArgs<T> a)
 {
     asm volatile("griddepcontrol.launch_dependents;");   // see step_kernel
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const CellState cs = cell_state(a.code, a.mask, i, a.g.n);
+    const CellState cs = cell_state(a, i, a.g.n);
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (!cs.active) return;
     static_for<G>([&](auto gc) {
@@ -491,7 +505,7 @@ __global__ void macroscopic_kernel(const T* __restrict__ pop, const uint8_t* __r
 {
     constexpr bool SHIFT = sizeof(T) == 4;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const CellState cs = cell_state(code, a.mask, i, g.n);
+    const CellState cs = cell_state(a, i, g.n);
     if (i >= g.n) return;
     T r = T(0), uu[3] = {T(0), T(0), T(0)};
     if (cs.active) {
@@ -514,7 +528,7 @@ __global__ void __launch_bounds__(256, sizeof(T) == 8 ? (Q == 19 ? 3 : 2) : (Q =
     constexpr bool SHIFT = sizeof(T) == 4;
     double e = 0.0;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    const CellState cs = cell_state(code, a.mask, i, g.n);
+    const CellState cs = cell_state(a, i, g.n);
     if (cs.active) {
         T f[Q], r, dr, uu[3];
         load_cell<T, Q, SOA, LOAD>(a, i, cs.masked, cs.mask, f);
@@ -579,24 +593,86 @@ __global__ void insert_plane_kernel(T* __restrict__ pop, const uint8_t* __restri
 }
 
 // halo exchange of the slab decomposition along x: one x-layer (ny*nz contiguous
-// cells in SoA) of the `ndir` population planes listed in p.dir, to (PACK) or from a contiguous
-// buffer [ndir][ny*nz].  Raw stored values (fp32: shifted), so both ends must have the same dtype.
+// cells in SoA) of `ndir` population planes to (PACK) or from a contiguous buffer [ndir][ny*nz].
+// Raw stored values (fp32: shifted), so both ends must have the same dtype.
+//
+//   slot[d]     population plane of the d-th direction of the message (k, or kbar where the scheme
+//               keeps post-collision values in the opposite slot: AA even, swap pass 1)
+//   first       index of the first cell of the layer read (PACK) or written (unpack)
+//   merge != 0  (unpack only) the message holds values that a neighbouring slab would have pushed or
+//               exchanged into this slab's outermost OWNED layer (AA odd step, swap pass 2): cell x
+//               of that layer takes direction d only when its upstream cell x - c_d, which lies in
+//               the ghost layer starting at `up_first`, is a GHOST cell (fluid on the neighbour); a
+//               solid upstream cell means x has bounced that population back itself.
+//               merge == 1: the buffer is indexed by the destination cell, == 2: by the upstream cell.
+//   flag        PACK: when not null the buffer is the RECEIVE buffer of the neighbouring slab (peer
+//               memory, written over NVLink), and the block that finishes last publishes `seq`
+//               there with system scope; unpack: when not null, wait until *flag >= seq first.
 struct HaloArgs {
-    int dir[9];
+    int slot[9];
+    int cy[9], cz[9];
     int ndir;
-    long long first;   // index of the first cell of the layer
+    long long first, up_first;
+    int ny, nz;
     int cells;         // ny*nz
+    int merge;
+    unsigned long long* flag;
+    unsigned long long seq;
+    unsigned* counter;   // PACK + flag: blocks done so far (sender's memory, zero between launches)
+    int* status;         // unpack + flag: set to 1 when the wait gave up
 };
+__device__ __forceinline__ unsigned long long ld_acquire_sys(const unsigned long long* p)
+{
+    unsigned long long v;
+    asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
 template <class T, bool PACK>
-__global__ void halo_kernel(T* __restrict__ pop, long long stride, HaloArgs p, T* __restrict__ buf)
+__global__ void __launch_bounds__(256) halo_kernel(T* __restrict__ pop, const uint8_t* __restrict__ code, long long stride,
+                                                   HaloArgs p, T* __restrict__ buf)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t >= p.cells) return;
     const int d = blockIdx.y;
-    T* slot = pop + (long long)p.dir[d] * stride + p.first + t;
-    T* b = buf + (long long)d * p.cells + t;
-    if (PACK) *b = *slot;
-    else *slot = *b;
+    if (!PACK && p.flag) {   // the message must have landed (bounded wait: a lost neighbour must not hang the GPU)
+        __shared__ int ok;
+        if (threadIdx.x == 0) {
+            int good = 0;
+            for (long long spin = 0; spin < (1LL << 24); ++spin) {
+                if (ld_acquire_sys(p.flag) >= p.seq) { good = 1; break; }
+                __nanosleep(64);
+            }
+            if (!good) *p.status = 1;
+            ok = good;
+        }
+        __syncthreads();
+        if (!ok) return;
+    }
+    if (t < p.cells) {
+        T* b = buf + (long long)d * p.cells + t;
+        T* slot = pop + (long long)p.slot[d] * stride + p.first + t;
+        if (PACK) {
+            *b = *slot;
+        } else if (!p.merge) {
+            *slot = *b;
+        } else {
+            const int iy = t / p.nz, iz = t - iy * p.nz;
+            const int up = wrap1(iy - p.cy[d], p.ny) * p.nz + wrap1(iz - p.cz[d], p.nz);
+            if (code[p.up_first + up] == CODE_GHOST && !(code[p.first + t] & 3))
+                *slot = buf[(long long)d * p.cells + (p.merge == 2 ? up : t)];
+        }
+    }
+    if (PACK && p.flag) {   // publish: every block's stores first, then the sequence number
+        __threadfence_system();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned total = gridDim.x * gridDim.y;
+            if (atomicAdd(p.counter, 1u) == total - 1u) {
+                *p.counter = 0u;
+                __threadfence_system();
+                asm volatile("st.release.sys.global.u64 [%0], %1;" ::"l"(p.flag), "l"(p.seq) : "memory");
+            }
+        }
+    }
 }
 
 }  // namespace lbm

@@ -9,15 +9,25 @@ first and last layer stand for the neighbours' nearest layers: LBM_GHOST where t
 bounce-back at a wall owned by another rank needs no communication).  The ranks form a ring, which is
 the periodic wrap of the library's index arithmetic; a cavity simply has walls at both ends of it.
 
-After every time step each rank sends, per face, the post-collision populations that leave through
-it (5 of 19 planes, 9 of 27) and receives the ones that enter: `lbm_halo_pack` -> send/recv ->
-`lbm_halo_unpack` (include/lbm.h).  That exchange is the only data-path communication; the kinetic
-energy adds one scalar all-reduce.  Two-population SoA scheme (pull form) only.
+Every time step each rank sends, per face, the populations that cross it (5 of 19 planes, 9 of 27)
+and receives the ones that enter; what exactly a message holds depends on the scheme (two-population:
+post-collision values pulled by the next step; AA: post-collision values after an even step, pushed
+values merged on arrival after an odd step; swap: between pass 1 and pass 2) and is the library's
+business (include/lbm.h).  The step runs in parts so that the transfer overlaps the interior update:
+begin (outermost owned layers) -> pack -> end (interior) -> unpack -> finish.  That exchange is the
+only data-path communication; the kinetic energy adds one scalar all-reduce.  SoA schemes only.
+
+Two transports:
+  * "peer": the library's own driver (`lbm_slab_step`): pack kernels store straight into the
+    neighbouring slab's receive buffer (peer memory over NVLink) and publish a sequence number, unpack
+    kernels wait for it; no host code and no communication library between the parts.  Slabs of one
+    process are linked directly (`lbm_slab_link`), slabs of other processes through CUDA IPC handles
+    exchanged once at start-up.
+  * "p2p": pack -> torch.distributed isend / irecv (NCCL on GPUs; gloo with CPU buffers in the host
+    tests) -> unpack, driven from Python once per step.
 
 This module holds the decomposition arithmetic and the exchange plumbing, no arithmetic of the
-method.  `exchange_local` serves several slabs living in one process (how the 1-GPU tests check the
-halo kernels against the oracle); `exchange_dist` is the one-process-per-GPU path over
-torch.distributed (NCCL on GPUs; the same code runs over gloo with CPU buffers in the host tests).
+method.
 """
 import numpy as np
 
@@ -95,7 +105,7 @@ def exchange_local(engines):
 def exchange_start(engine, dist, rank, world, group=None):
     """pack both faces and post the sends / receives; returns a handle for exchange_finish.  Over
     nccl the transfers run on the communicator's own stream, so whatever the caller launches next
-    on the compute stream (lbm_step_end: the interior of the slab) overlaps them."""
+    on the compute stream (step_end: the interior of the slab) overlaps them."""
     s0, s1 = engine.halo_pack(0), engine.halo_pack(1)
     r0, r1 = engine.halo_recv_buffer(0), engine.halo_recv_buffer(1)
     if world == 1:
@@ -125,11 +135,37 @@ def exchange_dist(engine, dist, rank, world, group=None):
     exchange_finish(engine, exchange_start(engine, dist, rank, world, group))
 
 
-def step_local(engines, overlap=True):
-    """one time step of several GPU slabs living in this process.  overlap = the order a multi-GPU
-    run uses: outer layers, pack, interior, unpack (lbm_step_begin / lbm_step_end)."""
+def step_dist(engine, dist, rank, world, group=None):
+    """one time step of one slab per process over torch.distributed: the parts in the order every
+    scheme needs (swap: the halo must arrive between pass 1 and pass 2)"""
+    engine.step_begin()                                  # the two outermost owned layers
+    h = exchange_start(engine, dist, rank, world, group)
+    engine.step_end()                                    # the interior, while the halo travels
+    exchange_finish(engine, h)
+    engine.step_finish()
+
+
+def link_ring(engines):
+    """link the slabs of this process into the periodic ring (library transport, lbm_slab_link)"""
     W = len(engines)
-    if overlap:
+    for r, e in enumerate(engines):
+        left, right = neighbours(r, W)
+        e.lbm.slab_link(0, engines[left].lbm)
+        e.lbm.slab_link(1, engines[right].lbm)
+
+
+def step_local(engines, mode="overlap"):
+    """one time step of several GPU slabs living in this process (one stream).
+    "overlap": outer layers, pack, interior, unpack, finish through the halo calls, buffers handed
+    over directly; "plain": lbm_step(1) then the exchange (two-population and AA only); "peer": the
+    library's driver after link_ring (post on all slabs, then complete on all)."""
+    W = len(engines)
+    if mode == "peer":
+        for e in engines:
+            e.lbm.slab_post()
+        for e in engines:
+            e.lbm.slab_complete()
+    elif mode == "overlap":
         for e in engines:
             e.lbm.step_begin()
         sent = [(e.halo_pack(0), e.halo_pack(1)) for e in engines]
@@ -139,6 +175,8 @@ def step_local(engines, overlap=True):
             left, right = neighbours(r, W)
             e.halo_unpack(0, sent[left][1])
             e.halo_unpack(1, sent[right][0])
+        for e in engines:
+            e.lbm.step_finish()
     else:
         for e in engines:
             e.lbm.step(1)
@@ -146,14 +184,17 @@ def step_local(engines, overlap=True):
 
 
 class GpuSlabEngine:
-    """one slab on the current CUDA device: an Lbm context plus its four halo buffers"""
+    """one slab on the current CUDA device: an Lbm context plus its four halo buffers.  Everything the
+    engine launches or copies goes to the stream that was current when it was built (the context's)."""
 
-    def __init__(self, flags_local, u_wall, lattice=19, collision="BGK_W2", omega=1.0, dtype="f64"):
+    def __init__(self, flags_local, u_wall, lattice=19, collision="BGK_W2", omega=1.0, dtype="f64", scheme="2POP_SOA"):
         import torch
         from .binding import Lbm, NP_DTYPES
         nx, ny, nz = flags_local.shape
         self.shape = (nx, ny, nz)
-        self.lbm = Lbm(nx, ny, nz, lattice=lattice, collision=collision, scheme="2POP_SOA", omega=omega, dtype=dtype)
+        self._torch = torch
+        self._stream = torch.cuda.current_stream()
+        self.lbm = Lbm(nx, ny, nz, lattice=lattice, collision=collision, scheme=scheme, omega=omega, dtype=dtype)
         self.lbm.set_flags(flags_local, u_wall)
         tdt = torch.float64 if dtype == "f64" else torch.float32
         self.np_dtype = NP_DTYPES[dtype]
@@ -161,6 +202,15 @@ class GpuSlabEngine:
         self._send = [torch.empty(cnt, dtype=tdt, device="cuda") for _ in range(2)]
         self._recv = [torch.empty(cnt, dtype=tdt, device="cuda") for _ in range(2)]
         self.halo_bytes = 2 * cnt * self._send[0].element_size()  # sent per step (received: the same)
+
+    def step_begin(self):
+        self.lbm.step_begin()
+
+    def step_end(self):
+        self.lbm.step_end()
+
+    def step_finish(self):
+        self.lbm.step_finish()
 
     def halo_pack(self, face):
         self.lbm.halo_pack(face, self._send[face].data_ptr())
@@ -171,6 +221,10 @@ class GpuSlabEngine:
 
     def halo_unpack(self, face, buf):
         self.lbm.halo_unpack(face, buf.data_ptr())
+
+    def on_stream(self):
+        """context manager: torch work (copies, NCCL transfers) ordered on the context's stream"""
+        return self._torch.cuda.stream(self._stream)
 
     def close(self):
         self.lbm.close()
@@ -183,11 +237,15 @@ class SlabLbm:
     (kinetic energy)."""
 
     def __init__(self, NX, NY, NZ, flags=None, u_wall=(0.0, 0.0, 0.0), dist=None, rank=0, world=1, group=None,
-                 lattice=19, collision="BGK_W2", omega=1.0, dtype="f64", flags_local=None, overlap=True):
+                 lattice=19, collision="BGK_W2", omega=1.0, dtype="f64", flags_local=None, scheme="2POP_SOA",
+                 transport=None):
         """flags: GLOBAL [NX, NY, NZ] (None = all fluid), or flags_local: this rank's [nxl+2, NY, NZ]
-        with its ghost layers already in place (local_flags / cavity_slab)"""
-        self.dist, self.rank, self.world, self.group = dist, rank, world, group
-        self.overlap = overlap    # exchange the halo while the interior of the slab is updated
+        with its ghost layers already in place (local_flags / cavity_slab).
+        transport: "peer" (library driver over peer memory; default for one rank) or "p2p"
+        (torch.distributed send / recv; default for several ranks)"""
+        self.dist, self.rank, self.group = dist, rank, group
+        self.world = world if dist is not None else 1
+        self.transport = transport or ("peer" if self.world == 1 else "p2p")
         self.N = (NX, NY, NZ)
         self.x0, self.x1 = slab_range(NX, rank, world)
         if flags_local is not None:
@@ -196,9 +254,26 @@ class SlabLbm:
             if flags is None:
                 flags = np.zeros((NX, NY, NZ), dtype=np.uint8)
             self.flags_local = local_flags(np.asarray(flags).reshape(NX, NY, NZ), self.x0, self.x1)
-        self.engine = GpuSlabEngine(self.flags_local, u_wall, lattice=lattice, collision=collision, omega=omega, dtype=dtype)
+        self.engine = GpuSlabEngine(self.flags_local, u_wall, lattice=lattice, collision=collision, omega=omega,
+                                    dtype=dtype, scheme=scheme)
         self.lbm = self.engine.lbm
         self.Q = self.lbm.Q
+        if self.transport == "peer":
+            self._connect_peers()
+
+    def _connect_peers(self):
+        """library transport: one slab = the ring closes on itself; several processes = every rank
+        publishes the CUDA IPC handle of its receive block and opens its two neighbours' """
+        if self.world == 1:
+            self.lbm.slab_link(0, self.lbm)
+            self.lbm.slab_link(1, self.lbm)
+            return
+        handles = [None] * self.world
+        self.dist.all_gather_object(handles, self.lbm.slab_export(), group=self.group)
+        left, right = neighbours(self.rank, self.world)
+        self.lbm.slab_import(0, handles[left])
+        self.lbm.slab_import(1, handles[right])
+        self.dist.barrier(group=self.group)
 
     def _local(self, a, lead):
         NX, NY, NZ = self.N
@@ -213,16 +288,12 @@ class SlabLbm:
         self.lbm.init_equilibrium(np.asarray(rho_local, dtype=self.engine.np_dtype), np.asarray(u_local, dtype=self.engine.np_dtype))
 
     def step(self, n=1):
-        world = self.world if self.dist is not None else 1
-        for _ in range(n):
-            if self.overlap:
-                self.lbm.step_begin()                       # the two outermost owned layers
-                h = exchange_start(self.engine, self.dist, self.rank, world, self.group)
-                self.lbm.step_end()                         # the interior, while the halo travels
-                exchange_finish(self.engine, h)
-            else:
-                self.lbm.step(1)
-                exchange_dist(self.engine, self.dist, self.rank, world, self.group)
+        if self.transport == "peer":
+            self.lbm.slab_step(n)       # the whole loop inside the library, nothing per step on the host
+            return
+        with self.engine.on_stream():
+            for _ in range(n):
+                step_dist(self.engine, self.dist, self.rank, self.world, self.group)
 
     def macroscopic(self):
         """(rho [nxl, NY, NZ], u [3, nxl, NY, NZ]) of the owned layers"""
@@ -236,18 +307,20 @@ class SlabLbm:
         return interior(self.lbm.get_populations().reshape(self.Q, nx, ny, nz), axis=1).copy()
 
     def kinetic_energy(self):
-        """global sum (one scalar all-reduce)"""
-        e = self.lbm.kinetic_energy()
-        if self.dist is not None and self.world > 1:
-            import torch
-            t = torch.tensor([e], dtype=torch.float64, device="cuda")
-            self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
-            e = float(t.item())
-        return e
+        """global sum: the slab's partial stays in device memory for the one scalar all-reduce"""
+        import torch
+        with self.engine.on_stream():
+            t = torch.zeros(1, dtype=torch.float64, device="cuda")
+            self.lbm.kinetic_energy_device(t.data_ptr())
+            if self.dist is not None and self.world > 1:
+                self.dist.all_reduce(t, op=self.dist.ReduceOp.SUM, group=self.group)
+            return float(t.item())
 
     @property
     def num_fluid(self):
         return self.lbm.num_fluid
 
     def close(self):
+        if self.transport == "peer":
+            self.lbm.slab_status()
         self.engine.close()
