@@ -115,8 +115,12 @@ long long lbm_device_bytes(const lbm_t* ctx);
 long long lbm_kernel_launches(const lbm_t* ctx);
 /* Block until everything queued on the context's stream has finished. */
 int lbm_sync(lbm_t* ctx);
-/* Select an implementation variant of the step kernels (0 = default); used by the bench sweep.
- * Unknown variants return LBM_E_ARG.  Results are identical across variants. */
+/* Select an implementation variant of the step kernels; results are identical across variants
+ * (tests compare them bit for bit).  0 default (library's choice); 1 generic_push: two-population as
+ * the paper's collide-then-push (Table 1); 2 generic_pull: as pull-then-collide with
+ * lazily streamed storage (the default); 3 aos_plain: AoS without the shared-memory tile; 4 tma: SoA
+ * loads staged through shared memory by TMA bulk copies; 5 no_tma: never that kernel; 6 plain:
+ * one cell per thread, no L2 prefetch, no programmatic dependent launch.  Unknown: LBM_E_ARG. */
 int lbm_set_variant(lbm_t* ctx, int variant);
 
 /* Threads per block of the step kernels (tuning knob of the sweep; multiple of 32 in [32, 256];
@@ -194,11 +198,6 @@ int lbm_slab_status(lbm_t* ctx);
 enum { LBM_GRAPH_AUTO = 0, LBM_GRAPH_OFF = 1, LBM_GRAPH_ON = 2 };
 int lbm_set_graph(lbm_t* ctx, int mode);
 long long lbm_graph_replays(const lbm_t* ctx);
-
-/* Tuning knobs read from the environment by lbm_create (results never depend on them):
- *   LBM_PF=<cells>  distance of the L2 prefetch the step kernels issue ahead of the block scheduler
- *                   (default 16384 cells in fp64, 65536 in fp32; 0 = off; only lattices beyond L2);
- *   LBM_PDL=0       no programmatic dependent launch of the step kernels. */
 
 const char* lbm_last_error(void);
 const char* lbm_version(void);

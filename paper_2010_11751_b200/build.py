@@ -55,11 +55,7 @@ def jobs():
     return out
 
 
-def build(force: bool = False, verbose: bool = False, defines=(), out: str = None) -> str:
-    """defines / out: build a tuning variant (extra -D flags) into another file; the default build
-    ignores them."""
-    if out is not None:
-        return _build_variant(list(defines), out)
+def build(force: bool = False, verbose: bool = False) -> str:
     stamp_file = os.path.join(OBJ, "stamp.txt")
     stamp = _stamp()
     if not force and os.path.exists(LIB) and os.path.exists(stamp_file) and open(stamp_file).read() == stamp:
@@ -81,21 +77,5 @@ def build(force: bool = False, verbose: bool = False, defines=(), out: str = Non
     return LIB
 
 
-def _build_variant(defines, out):
-    """same sources with extra -D flags, objects in a directory of their own"""
-    obj_dir = out + ".obj"
-    os.makedirs(obj_dir, exist_ok=True)
-    todo = [(src, os.path.join(obj_dir, os.path.basename(obj)), defs + ["-D" + d for d in defines]) for src, obj, defs in jobs()]
-    with cf.ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
-        for f in [ex.submit(_run, ["nvcc"] + NVCC_FLAGS + defs + ["-c", src, "-o", obj]) for src, obj, defs in todo]:
-            f.result()
-    _run(["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", out] + [obj for _, obj, _ in todo])
-    return out
-
-
 if __name__ == "__main__":
-    if "--out" in sys.argv:
-        defs = [a[2:] for a in sys.argv if a.startswith("-D")]
-        print(build(defines=defs, out=sys.argv[sys.argv.index("--out") + 1]))
-        sys.exit(0)
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

@@ -56,8 +56,9 @@ def steady_cavity_profiles(n, re=1000.0, u_lb=0.06, max_turnovers=100.0, tol=1e-
         max_steps = int(max_turnovers * (n - 2) / u_lb)
         history, steps, e_prev, change = [], 0, None, None
         while steps < max_steps:
-            g.step(check_every)
-            steps += check_every
+            chunk = min(check_every, max_steps - steps)
+            g.step(chunk)
+            steps += chunk
             e = g.kinetic_energy()
             if not np.isfinite(e):
                 raise RuntimeError("cavity run blew up at step %d" % steps)

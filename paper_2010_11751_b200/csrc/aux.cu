@@ -277,9 +277,10 @@ LBM_AUX_INST(float)
 LBM_AUX_INST(double)
 
 template <int Q>
-static void tables_of(int (*c)[3], int* opp, double* w)
+static void tables_of(int (*c)[3], int* opp, double* w, int* aos)
 {
     for (int k = 0; k < Q; ++k) {
+        aos[k] = Lat<Q>::aos_slot(k);
         c[k][0] = Lat<Q>::cx(k);
         c[k][1] = Lat<Q>::cy(k);
         c[k][2] = Lat<Q>::cz(k);
@@ -287,10 +288,10 @@ static void tables_of(int (*c)[3], int* opp, double* w)
         w[k] = Lat<Q>::w(k);
     }
 }
-void lattice_tables(int Q, int (*c)[3], int* opp, double* w)
+void lattice_tables(int Q, int (*c)[3], int* opp, double* w, int* aos)
 {
-    if (Q == 19) tables_of<19>(c, opp, w);
-    else tables_of<27>(c, opp, w);
+    if (Q == 19) tables_of<19>(c, opp, w, aos);
+    else tables_of<27>(c, opp, w, aos);
 }
 
 }  // namespace lbm

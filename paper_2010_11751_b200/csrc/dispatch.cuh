@@ -24,6 +24,7 @@ enum Variant {
     V_AOS_PLAIN,     // AoS without the shared-memory tile (every access a per-thread gather / scatter)
     V_TMA,           // SoA: loads staged through shared memory by TMA bulk copies (tma_step.cuh)
     V_NO_TMA,        // SoA: never that kernel (one cell per thread, loads into registers, L2 prefetch)
+    V_PLAIN,         // as V_NO_TMA, and neither L2 prefetch nor programmatic dependent launch (pure scheduling: same results)
     V_COUNT
 };
 
@@ -60,7 +61,7 @@ cudaError_t aux_halo(bool pack, T* pop, const uint8_t* code, long long stride, c
 template <class T>
 cudaError_t aux_stream_only(int Q, bool soa, const StepArgs<T>& a, cudaStream_t s);
 
-// host copies of the lattice tables (from Lat<Q>)
-void lattice_tables(int Q, int (*c)[3], int* opp, double* w);
+// host copies of the lattice tables (from Lat<Q>); aos[k] = slot of direction k inside an AoS record
+void lattice_tables(int Q, int (*c)[3], int* opp, double* w, int* aos);
 
 }  // namespace lbm

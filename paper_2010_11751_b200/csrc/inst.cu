@@ -16,7 +16,7 @@ static cudaError_t launch_one(int block, bool staged, const StepArgs<T>& a, cuda
     if constexpr (!SOA && (LOAD == LD_LOCAL || STORE != ST_PUSH)) {
         if (staged && a.first == 0 && a.end == a.g.n) {  // AoS: local accesses through a transposing shared-memory tile (kernels.cuh)
             const int b = block > 128 ? 128 : block;
-            step_kernel_aos<T, Q, MODEL, LOAD, STORE><<<(a.g.n + b - 1) / b, b, (size_t)b * Q * sizeof(T), s>>>(a);
+            step_kernel_aos<T, Q, MODEL, LOAD, STORE><<<(a.g.n + b - 1) / b, b, ((size_t)b * Q + (size_t)(b / 32) * 96) * sizeof(T), s>>>(a);
             return cudaGetLastError();
         }
     }

@@ -73,12 +73,32 @@ struct StepArgs {
     //   wso[k]    byte offset of the slot the masked ST_PUSH store of f_k writes when the
     //             downstream cell is solid: plane[kbar]
     long long plane[27], ldo[27], sto[27], wlo[27], wso[27];
+    // SoA: the same as pointers, lp[k] = src + ldo[k], sp[k] = dst + sto[k] (in elements), so that the
+    // pure access of cell i is lp[k][i] with a 32-bit i: one IMAD.WIDE with the pointer taken from the
+    // constant bank instead of a 64-bit add in two instructions (57 fewer integer instructions per
+    // D3Q19 cell: the fp32 kernels are close to issue-bound)
+    const T* lp[27];
+    T* sp[27];
 };
 
+// element index of STORAGE slot s of cell i (SoA: plane s; AoS: s-th value of the record)
 template <bool SOA, int Q>
-__device__ __forceinline__ long long slot(const Geo& g, int k, long long i)
+__device__ __forceinline__ long long slot_raw(const Geo& g, int s, long long i)
 {
-    return SOA ? (long long)k * g.stride + i : i * Q + k;
+    return SOA ? (long long)s * g.stride + i : i * Q + s;
+}
+// storage slot of direction K: K itself in SoA, Lat<Q>::aos_slot(K) in AoS
+template <bool SOA, int Q, int K>
+__host__ __device__ constexpr int storage_slot()
+{
+    return SOA ? K : Lat<Q>::aos_slot(K);
+}
+// element index of direction K (compile-time) of cell i
+template <bool SOA, int Q, int K>
+__device__ __forceinline__ long long slot(const Geo& g, long long i)
+{
+    constexpr int s = storage_slot<SOA, Q, K>();
+    return slot_raw<SOA, Q>(g, s, i);
 }
 
 __device__ __forceinline__ int wrap1(int v, int n) { return v < 0 ? v + n : (v >= n ? v - n : v); }
@@ -149,8 +169,12 @@ __device__ __forceinline__ void load_cell(const StepArgs<T>& a, int i, bool mask
     constexpr int IS = SOA ? 1 : Q;
     const T* __restrict__ src = a.src;
     if (LOAD == LD_LOCAL || !masked) {
-        const char* __restrict__ p = reinterpret_cast<const char*>(src + (long long)i * IS);
-        static_for<Q>([&](auto kc) { f[kc] = *reinterpret_cast<const T*>(p + a.ldo[kc]); });
+        if constexpr (SOA) {
+            static_for<Q>([&](auto kc) { f[kc] = a.lp[kc][i]; });
+        } else {
+            const char* __restrict__ p = reinterpret_cast<const char*>(src + (long long)i * IS);
+            static_for<Q>([&](auto kc) { f[kc] = *reinterpret_cast<const T*>(p + a.ldo[kc]); });
+        }
     } else {
         const Edge e(mask, a.g);
         const char* __restrict__ p = reinterpret_cast<const char*>(src + (long long)i * IS);
@@ -176,8 +200,12 @@ __device__ __forceinline__ void store_cell(const StepArgs<T>& a, int i, bool mas
     constexpr int IS = SOA ? 1 : Q;
     T* __restrict__ dst = a.dst;
     if (STORE != ST_PUSH || !masked) {
-        char* __restrict__ p = reinterpret_cast<char*>(dst + (long long)i * IS);
-        static_for<Q>([&](auto kc) { *reinterpret_cast<T*>(p + a.sto[kc]) = f[kc]; });
+        if constexpr (SOA) {
+            static_for<Q>([&](auto kc) { a.sp[kc][i] = f[kc]; });
+        } else {
+            char* __restrict__ p = reinterpret_cast<char*>(dst + (long long)i * IS);
+            static_for<Q>([&](auto kc) { *reinterpret_cast<T*>(p + a.sto[kc]) = f[kc]; });
+        }
     } else {
         const Edge e(mask, a.g);
         char* __restrict__ p = reinterpret_cast<char*>(dst + (long long)i * IS);
@@ -275,8 +303,12 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
         // a DRAM read-modify-write when it is evicted (ncu: +80 MB read per 256^3 step, both precisions)
         if constexpr (STORE == ST_LOCAL && LOAD != LD_LOCAL) {
             if (cs.partial) {
-                char* __restrict__ p = reinterpret_cast<char*>(a.dst + (long long)i * (SOA ? 1 : Q));
-                static_for<Q>([&](auto kc) { *reinterpret_cast<T*>(p + a.sto[kc]) = T(0); });
+                if constexpr (SOA) {
+                    static_for<Q>([&](auto kc) { a.sp[kc][i] = T(0); });
+                } else {
+                    char* __restrict__ p = reinterpret_cast<char*>(a.dst + (long long)i * Q);
+                    static_for<Q>([&](auto kc) { *reinterpret_cast<T*>(p + a.sto[kc]) = T(0); });
+                }
             }
         }
         return;
@@ -298,16 +330,21 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
         if (!a.pf_strided) {
             const long long t = (long long)i + a.pf;   // 64-bit: N may be close to 2^31
             if (t >= margin && t + margin < a.g.n && t < a.end) {
-                const char* q = reinterpret_cast<const char*>(a.src + t * (SOA ? 1 : Q));
-                static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(q + a.ldo[kc])); });
+                if constexpr (SOA) {
+                    const int ti = (int)t;
+                    static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a.lp[kc] + ti)); });
+                } else {
+                    const char* q = reinterpret_cast<const char*>(a.src + t * Q);
+                    static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(q + a.ldo[kc])); });
+                }
             }
         } else if constexpr (SOA) {
             constexpr int CPL = 128 / sizeof(T);   // cells per line
             const int lane = threadIdx.x & 31;
             const long long tgt = (long long)(i - lane) + a.pf + (long long)lane * CPL;
             if ((((i - a.first) >> 5) % CPL) == 0 && tgt >= margin && tgt + CPL + margin < a.g.n && tgt + CPL < a.end) {
-                const char* q = reinterpret_cast<const char*>(a.src + tgt);
-                static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(q + a.ldo[kc])); });
+                const int ti = (int)tgt;
+                static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a.lp[kc] + ti)); });
             }
         }
     }
@@ -317,36 +354,125 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
     store_cell<T, Q, SOA, STORE>(a, i, cs.masked, cs.mask, f);
 }
 
+// AoS, neighbour side.  A warp that pulls "slot k of 32 consecutive cells" touches 32 different 32-byte
+// sectors and uses 4 or 8 bytes of each; ncu (profiles/r02_aos_*) shows the AoS gathers running at the
+// rate the LSU / L2 deliver such sectors, not at the DRAM rate.  The internal slot order of a record
+// (Lat<Q>::aos_slot) puts the three directions that share (cx, cy) next to each other, so the values a
+// warp of bulk cells pulls from ONE neighbouring z-row are the adjacent triples (cz = -1, 0, +1) of 32
+// consecutive records: lane l needs slot 1 + s*dz of record l - dz (s = +1 pull, -1 AA pull).  The
+// warp therefore loads those 96 values with three requests in which consecutive lanes read consecutive
+// addresses (lane -> (record e/3, slot e%3), e = 32j + lane: 11-14 sectors per request instead of
+// 32, every byte used), parks them in 96 elements of shared memory and each lane picks its three; only
+// the two values that come from the records beyond the ends of the run (lane 0: record -1, lane 31:
+// record 32) are fetched directly.  Directions alone in their (cx, cy) group (D3Q19: cz = 0 diagonals)
+// are loaded per thread as before.  Every lane of the warp must call this (bulk warps only).
+template <class T, int Q, int LOAD>
+__device__ __forceinline__ void load_cell_aos_coop(const StepArgs<T>& a, int i, T* __restrict__ scratch, T (&f)[Q])
+{
+    static_assert(LOAD == LD_PULL || LOAD == LD_AAPULL, "neighbour loads only");
+    using L = Lat<Q>;
+    const int lane = threadIdx.x & 31;
+    const T* __restrict__ src = a.src;
+    const long long b = (long long)i - lane;   // first cell of the warp
+    const long long A = (long long)a.g.ny * a.g.nz;
+    static_for<9>([&](auto gc) {
+        constexpr int gx = gc / 3 - 1, gy = gc % 3 - 1;
+        // directions of this (cx, cy) group, by cz
+        constexpr int km = L::dir_of_code((gx + 1) * 9 + (gy + 1) * 3 + 0);
+        constexpr int k0 = L::dir_of_code((gx + 1) * 9 + (gy + 1) * 3 + 1);
+        constexpr int kp = L::dir_of_code((gx + 1) * 9 + (gy + 1) * 3 + 2);
+        const long long R0 = b - (gx * A + gy * (long long)a.g.nz);   // record that lane 0 pulls its cz = 0 value from
+        if constexpr (km >= 0 && kp >= 0) {
+            // the triple lives in the group (gx, gy) of the source record (pull) or in (-gx, -gy) (AA pull: slot kbar)
+            constexpr int gs = LOAD == LD_PULL ? L::aos_slot(km) : L::aos_slot(L::opp(kp));
+            static_for<3>([&](auto jc) {
+                const int e = 32 * jc + lane, rec = e / 3, sl = e - 3 * rec;
+                scratch[e] = src[(R0 + rec) * Q + gs + sl];
+            });
+            __syncwarp();
+            static_for<3>([&](auto dc) {
+                constexpr int dz = dc - 1;
+                constexpr int k = dz < 0 ? km : dz == 0 ? k0 : kp;
+                constexpr int t = LOAD == LD_PULL ? 1 + dz : 1 - dz;
+                const int r = lane - dz;
+                T v;
+                if (r >= 0 && r < 32) v = scratch[3 * r + t];
+                else v = src[(R0 + r) * Q + gs + t];
+                f[k] = v;
+            });
+            __syncwarp();
+        } else if constexpr (k0 >= 0) {
+            constexpr int sl = LOAD == LD_PULL ? L::aos_slot(k0) : L::aos_slot(L::opp(k0));
+            f[k0] = src[(R0 + lane) * Q + sl];
+        }
+    });
+}
+
 // AoS with shared-memory staging.  In the AoS layout pop[N][Q] the Q values of
 // the cells of one block are one contiguous run of blockDim*Q elements, but a warp that reads
 // "slot k of 32 consecutive cells" touches 32 different sectors.  Whatever is LOCAL to the cell
 // (the loads of 2-pop push / AA even / swap pass 1 / collide-only, the stores of 2-pop pull /
-// AA even / swap pass 1 / collide-only) therefore goes through a transposing tile: the block
-// copies its run coalesced, each thread works on its own record tile[tid*Q .. tid*Q+Q) (Q is odd,
-// so both 4-byte and 8-byte records are free of bank conflicts).  Neighbour accesses (LD_PULL,
-// LD_AAPULL, ST_PUSH) stay per-thread gathers / scatters.  Launch with blockDim*Q*sizeof(T) bytes
-// of dynamic shared memory.
+// AA even / swap pass 1 / collide-only) therefore goes through a transposing tile: the run is copied
+// between global and shared memory by ONE 1-D TMA bulk copy each way (cp.async.bulk: no registers,
+// no per-thread address arithmetic, the whole run in flight at once; ncu showed the earlier
+// per-thread copy loop at half the bandwidth of the SoA kernels with 4 loads in flight per thread),
+// and each thread works on its own record tile[tid*Q .. tid*Q+Q) (Q is odd, so both 4-byte and
+// 8-byte records are free of bank conflicts).  Neighbour accesses (LD_PULL, LD_AAPULL, ST_PUSH) stay
+// per-thread gathers / scatters.  A run whose size is not a multiple of 16 bytes (the last block of
+// a ragged lattice) is copied by the threads.  Launch with (blockDim*Q + blockDim/32*96)*sizeof(T)
+// bytes of dynamic shared memory (the tile and the warps' gather scratch).
+__device__ __forceinline__ unsigned aos_smem_addr(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 template <class T, int Q, int MODEL, int LOAD, int STORE>
 __global__ void __launch_bounds__(128) step_kernel_aos(const StepArgs<T> a)
 {
     static_assert(LOAD == LD_LOCAL || STORE != ST_PUSH, "nothing to stage");
     constexpr bool SHIFT = sizeof(T) == 4;
     using L = Lat<Q>;
-    extern __shared__ __align__(16) unsigned char tile_raw[];
+    extern __shared__ __align__(128) unsigned char tile_raw[];
+    __shared__ __align__(8) unsigned long long bar;
     T* tile = reinterpret_cast<T*>(tile_raw);
     const long long base = (long long)blockIdx.x * blockDim.x;   // first cell of the block
     const int i = (int)base + threadIdx.x;
     const int nb = min((long long)blockDim.x, (long long)a.g.n - base) * Q;   // elements of the block's run
+    const unsigned bytes = (unsigned)nb * (unsigned)sizeof(T);
+    const bool bulk = (bytes & 15u) == 0u;   // base * Q * sizeof(T) is a multiple of 16 for blocks of 128 cells
+    if constexpr (LOAD == LD_LOCAL) {
+        if (bulk && threadIdx.x == 0) {
+            const unsigned b = aos_smem_addr(&bar);
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(b) : "memory");
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(b), "r"(bytes) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                         ::"r"(aos_smem_addr(tile)), "l"(a.src + base * Q), "r"(bytes), "r"(b) : "memory");
+        }
+    }
     const CellState cs = cell_state(a, i, a.g.n);
     T* rec = tile + threadIdx.x * Q;
     T f[Q];
     if constexpr (LOAD == LD_LOCAL) {
-        const T* __restrict__ run = a.src + base * Q;
-        for (int e = threadIdx.x; e < nb; e += blockDim.x) tile[e] = run[e];
-        __syncthreads();
-        if (cs.active) static_for<Q>([&](auto kc) { f[kc] = rec[kc]; });
+        if (bulk) {
+            __syncthreads();   // the barrier is initialised
+            const unsigned b = aos_smem_addr(&bar);
+            unsigned ok;
+            do {
+                asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0; selp.u32 %0, 1, 0, p; }"
+                             : "=r"(ok) : "r"(b) : "memory");
+            } while (!ok);
+        } else {
+            const T* __restrict__ run = a.src + base * Q;
+            for (int e = threadIdx.x; e < nb; e += blockDim.x) tile[e] = run[e];
+            __syncthreads();
+        }
+        if (cs.active) static_for<Q>([&](auto kc) { constexpr int sl = L::aos_slot(kc); f[kc] = rec[sl]; });
     } else {
-        if (cs.active) load_cell<T, Q, false, LOAD>(a, i, cs.masked, cs.mask, f);
+        // bulk warps gather cooperatively (load_cell_aos_coop), the others per thread
+        const bool coop = __all_sync(0xffffffffu, cs.active && !cs.masked);
+        if (coop) {
+            T* scratch = tile + (size_t)blockDim.x * Q + (threadIdx.x >> 5) * 96;
+            load_cell_aos_coop<T, Q, LOAD>(a, i, scratch, f);
+        } else if (cs.active) {
+            load_cell<T, Q, false, LOAD>(a, i, cs.masked, cs.mask, f);
+        }
         // the other array is written: solid cells of the run get zeros (never read)
         if (!cs.active) static_for<Q>([&](auto kc) { rec[kc] = T(0); });
     }
@@ -354,10 +480,21 @@ __global__ void __launch_bounds__(128) step_kernel_aos(const StepArgs<T> a)
     if constexpr (STORE == ST_PUSH) {
         if (cs.active) store_cell<T, Q, false, STORE>(a, i, cs.masked, cs.mask, f);
     } else {
-        if (cs.active) static_for<Q>([&](auto kc) { rec[STORE == ST_SWAPPED ? L::opp(kc) : (int)kc] = f[kc]; });
-        __syncthreads();
-        T* __restrict__ run = a.dst + base * Q;
-        for (int e = threadIdx.x; e < nb; e += blockDim.x) run[e] = tile[e];
+        if (cs.active) static_for<Q>([&](auto kc) { constexpr int sl = L::aos_slot(STORE == ST_SWAPPED ? L::opp(kc) : (int)kc); rec[sl] = f[kc]; });
+        if (bulk) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the records, written by the threads, are read by the TMA unit
+            __syncthreads();
+            if (threadIdx.x == 0) {
+                asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                             ::"l"(a.dst + base * Q), "r"(aos_smem_addr(tile)), "r"(bytes) : "memory");
+                asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the tile must outlive the copy
+            }
+        } else {
+            __syncthreads();
+            T* __restrict__ run = a.dst + base * Q;
+            for (int e = threadIdx.x; e < nb; e += blockDim.x) run[e] = tile[e];
+        }
     }
 }
 
@@ -404,15 +541,15 @@ __device__ __forceinline__ void swap_pairs(const StepArgs<T>& a, int i, const Ce
         static_for<L::NH>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
             if constexpr (k % G == GI) {
-                va[k] = pop[slot<SOA, Q>(g, kb, i)];
-                vb[k] = pop[slot<SOA, Q>(g, k, (long long)i + offset<Q, k>(g))];
+                va[k] = pop[slot<SOA, Q, kb>(g, i)];
+                vb[k] = pop[slot<SOA, Q, k>(g, (long long)i + offset<Q, k>(g))];
             }
         });
         static_for<L::NH>([&](auto kc) {
             constexpr int k = kc, kb = L::opp(k);
             if constexpr (k % G == GI) {
-                pop[slot<SOA, Q>(g, kb, i)] = vb[k];
-                pop[slot<SOA, Q>(g, k, (long long)i + offset<Q, k>(g))] = va[k];
+                pop[slot<SOA, Q, kb>(g, i)] = vb[k];
+                pop[slot<SOA, Q, k>(g, (long long)i + offset<Q, k>(g))] = va[k];
             }
         });
     } else {
@@ -424,8 +561,8 @@ __device__ __forceinline__ void swap_pairs(const StepArgs<T>& a, int i, const Ce
             constexpr int k = kc, kb = L::opp(k);
             if constexpr (k % G == GI) {
                 const bool sol = e.template solid_at<Q, k>();
-                const long long pb = sol ? slot<SOA, Q>(g, k, i) : slot<SOA, Q>(g, k, (long long)i + e.template off<Q, k, +1>(g));
-                va[k] = pop[slot<SOA, Q>(g, kb, i)];
+                const long long pb = sol ? slot<SOA, Q, k>(g, i) : slot<SOA, Q, k>(g, (long long)i + e.template off<Q, k, +1>(g));
+                va[k] = pop[slot<SOA, Q, kb>(g, i)];
                 vb[k] = pop[pb];
             }
         });
@@ -434,17 +571,17 @@ __device__ __forceinline__ void swap_pairs(const StepArgs<T>& a, int i, const Ce
             if constexpr (k % G == GI) {
                 const bool sol = e.template solid_at<Q, k>();
                 const bool back_moving = e.template moving_at<Q, kb>();   // neighbour at x - c_k
-                const long long pa = slot<SOA, Q>(g, kb, i);
+                const long long pa = slot<SOA, Q, kb>(g, i);
                 if (!sol) {
-                    const long long pb = slot<SOA, Q>(g, k, (long long)i + e.template off<Q, k, +1>(g));
+                    const long long pb = slot<SOA, Q, k>(g, (long long)i + e.template off<Q, k, +1>(g));
                     pop[pa] = vb[k];
                     pop[pb] = va[k];
                     // pop_k(x) belongs to the exchange of the cell at x - c_k unless that one is solid
-                    if (back_moving) pop[slot<SOA, Q>(g, k, i)] += a.wterm[kb];
+                    if (back_moving) pop[slot<SOA, Q, k>(g, i)] += a.wterm[kb];
                 } else {
                     // vb[k] holds pop_k(x) here
                     if (e.template moving_at<Q, k>()) pop[pa] = va[k] + a.wterm[k];
-                    if (back_moving) pop[slot<SOA, Q>(g, k, i)] = vb[k] + a.wterm[kb];
+                    if (back_moving) pop[slot<SOA, Q, k>(g, i)] = vb[k] + a.wterm[kb];
                 }
             }
         });
@@ -462,15 +599,35 @@ swap_stream_kernel(const StepArgs<T> a)
     if (!cs.active) return;
     static_for<G>([&](auto gc) {
         if (blockIdx.y == (unsigned)gc) {
-            if (a.pf > 0 && (long long)i + a.pf + (long long)a.g.ny * a.g.nz + a.g.nz + 1 < a.g.n) {  // L2 prefetch, see step_kernel (offsets of the half set point forward only)
-                using L = Lat<Q>;
-                static_for<L::NH>([&](auto kc) {
-                    constexpr int k = kc, kb = L::opp(k);
-                    if constexpr (k % G == gc) {
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(a.dst + slot<SOA, Q>(a.g, kb, (long long)i + a.pf)));
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(a.dst + slot<SOA, Q>(a.g, k, (long long)i + a.pf + offset<Q, k>(a.g))));
-                    }
-                });
+            // L2 prefetch, see step_kernel (offsets of the half set point forward only): per thread in fp64,
+            // one warp in 32 with a line per lane in fp32 (pass 2 in fp32 ran at 77 % of the copy rate with
+            // 18 prefetch instructions in every thread)
+            const long long reach = (long long)a.g.ny * a.g.nz + a.g.nz + 1;
+            if (a.pf > 0 && !a.pf_strided) {
+                if ((long long)i + a.pf + reach < a.g.n) {
+                    using L = Lat<Q>;
+                    static_for<L::NH>([&](auto kc) {
+                        constexpr int k = kc, kb = L::opp(k);
+                        if constexpr (k % G == gc) {
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.dst + slot<SOA, Q, kb>(a.g, (long long)i + a.pf)));
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.dst + slot<SOA, Q, k>(a.g, (long long)i + a.pf + offset<Q, k>(a.g))));
+                        }
+                    });
+                }
+            } else if (a.pf > 0) {
+                constexpr int CPL = 128 / sizeof(T);   // cells per line
+                const int lane = threadIdx.x & 31;
+                const long long tgt = (long long)(i - lane) + a.pf + (long long)lane * CPL;
+                if (((i >> 5) % CPL) == 0 && tgt + CPL + reach < a.g.n) {
+                    using L = Lat<Q>;
+                    static_for<L::NH>([&](auto kc) {
+                        constexpr int k = kc, kb = L::opp(k);
+                        if constexpr (k % G == gc) {
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.dst + slot<SOA, Q, kb>(a.g, tgt)));
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(a.dst + slot<SOA, Q, k>(a.g, tgt + offset<Q, k>(a.g))));
+                        }
+                    });
+                }
             }
             swap_pairs<T, Q, SOA, G, gc>(a, i, cs);
         }
@@ -495,7 +652,7 @@ __global__ void init_equilibrium_kernel(T* __restrict__ pop, const uint8_t* __re
         if constexpr (EXT) equilibrium_ext<Q, SHIFT>(r, uu, E);
         else equilibrium_w2<Q, SHIFT>(r, r - T(1), uu, E);
     }
-    static_for<Q>([&](auto kc) { pop[slot<SOA, Q>(g, kc, i)] = E[kc]; });
+    static_for<Q>([&](auto kc) { pop[slot<SOA, Q, kc>(g, i)] = E[kc]; });
 }
 
 // rho, u of the pre-collision state; LOAD says where that state lives
@@ -574,8 +731,8 @@ __global__ void extract_plane_kernel(const T* __restrict__ pop, const uint8_t* _
             n = (wrap1(x - p.sx, g.nx) * g.ny + wrap1(y - p.sy, g.ny)) * g.nz + wrap1(z - p.sz, g.nz);
         }
         const int nc = code[n] & 3;
-        if (nc == 0 || nc == CODE_GHOST) v = pop[slot<SOA, Q>(g, p.slot_fluid, n)];
-        else v = pop[slot<SOA, Q>(g, p.slot_wall, i)] + (nc == CODE_MOVING ? T(p.wterm) : T(0));
+        if (nc == 0 || nc == CODE_GHOST) v = pop[slot_raw<SOA, Q>(g, p.slot_fluid, n)];
+        else v = pop[slot_raw<SOA, Q>(g, p.slot_wall, i)] + (nc == CODE_MOVING ? T(p.wterm) : T(0));
         if (SHIFT) v += T(p.weight);
     }
     out[t] = v;
@@ -589,7 +746,7 @@ __global__ void insert_plane_kernel(T* __restrict__ pop, const uint8_t* __restri
     if (i >= g.n) return;
     T v = T(0);
     if (!(code[i] & 3)) v = SHIFT ? in[i] - T(weight) : in[i];
-    pop[slot<SOA, Q>(g, k, i)] = v;
+    pop[slot_raw<SOA, Q>(g, k, i)] = v;
 }
 
 // halo exchange of the slab decomposition along x: one x-layer (ny*nz contiguous

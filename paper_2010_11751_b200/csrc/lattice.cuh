@@ -64,6 +64,18 @@ struct Lat {
             if (code(k) == g) return k;
         return -1;
     }
+    // slot of direction k inside an AoS record (internal order, free by R7): directions sorted by their
+    // grid code, i.e. by (cx, cy) first and cz last, so that the (up to) three directions that share
+    // (cx, cy) sit next to each other in the order cz = -1, 0, +1.  The populations a cell pulls from
+    // one neighbouring z-row then form adjacent triples of consecutive records (kernels.cuh, cooperative
+    // AoS gather).  D3Q27: the grid code itself.
+    LBM_HD static constexpr int aos_slot(int k)
+    {
+        int r = 0;
+        for (int j = 0; j < Q; ++j)
+            if (code(j) < code(k)) ++r;
+        return r;
+    }
     // weight t_k
     LBM_HD static constexpr double w(int k)
     {

@@ -74,13 +74,14 @@ struct lbm_ctx {
     lbm_free_fn free_fn;
     cudaStream_t stream;
     int c[27][3], opp[27];
+    int sslot[27];   // storage slot of direction k: k in SoA, its place inside the record in AoS (lattice.cuh)
     double w[27];
     // CUDA-graph replay of lbm_step for launch-bound lattices (see step_graphed)
     int graph_mode;             // LBM_GRAPH_AUTO / OFF / ON
     cudaGraphExec_t graph_exec[2]; // GRAPH_STEPS steps starting from graph_sto[j] with pop[0] == graph_pop0[j]: one per
                                    // parity, so that lbm_step(17) called repeatedly does not re-capture every time
-    int prefetch;                // L2 prefetch distance of the step kernels in cells (LBM_PF in the environment overrides)
-    int pdl;                     // programmatic dependent launch of the step kernels (LBM_PDL=0 in the environment turns it off)
+    int prefetch;                // L2 prefetch distance of the step kernels in cells, -1 = the tuned distances, 0 = off (variant "plain")
+    int pdl;                     // programmatic dependent launch of the step kernels (off in variant "plain")
     int range_first, range_end;  // cells the next step launch covers (0, 0 = all); lbm_step_begin / lbm_step_end
     int mid_step;                // 0, 1 after lbm_step_begin, 2 after lbm_step_end (until lbm_step_finish)
     int halo_mode;               // HaloMode
@@ -168,8 +169,8 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
         if (k >= c->Q) continue;
         const int kb = c->opp[k];
         const long long off = ((long long)c->c[k][0] * c->ny + c->c[k][1]) * c->nz + c->c[k][2];
-        const long long pk = c->soa ? (long long)k * c->g.stride : k;
-        const long long pkb = c->soa ? (long long)kb * c->g.stride : kb;
+        const long long pk = c->soa ? (long long)k * c->g.stride : c->sslot[k];
+        const long long pkb = c->soa ? (long long)kb * c->g.stride : c->sslot[kb];
         a.plane[k] = pk;
         a.ldo[k] = (long long)sizeof(T) * (load == LD_LOCAL ? pk : load == LD_PULL ? pk - off * is : pkb - off * is);
         a.sto[k] = (long long)sizeof(T) * (store == ST_LOCAL ? pk : store == ST_SWAPPED ? pkb : pk + off * is);
@@ -178,6 +179,10 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
     }
     a.src = (const T*)src;
     a.dst = (T*)dst;
+    for (int k = 0; k < 27; ++k) {
+        a.lp[k] = a.src ? a.src + a.ldo[k] / (long long)sizeof(T) : nullptr;
+        a.sp[k] = a.dst ? a.dst + a.sto[k] / (long long)sizeof(T) : nullptr;
+    }
     a.code = c->code;
     a.grp = c->grp;
     a.mask = c->mask;
@@ -250,7 +255,7 @@ cudaError_t step_kind(lbm_ctx* c, int kind, const void* src, void* dst)
     StepArgs<T> a = make_args<T>(c, src, dst, load, store);
     // L2 prefetch ahead of the block scheduler (kernels.cuh) for the kernels of the steady state: per
     // thread in fp64, one warp in 32 with a line per lane in fp32; nothing when the populations fit
-    // in L2 anyway (48^3: -5 %, 64^3: -3 % with it).  LBM_PF=<cells> overrides the distance, 0 = off.
+    // in L2 anyway (48^3: -5 %, 64^3: -3 % with it).  The variant "plain" switches it off.
     const bool beyond_l2 = c->pop_elems * c->elem * (c->fam == FAM_2POP ? 2 : 1) > (size_t)100 << 20;
     if (c->soa && beyond_l2 && (kind == SK_EVEN || kind == SK_ODD || kind == SK_PULL)) {
         a.pf_strided = sizeof(T) == 4;
@@ -297,7 +302,7 @@ int swap_pass2(lbm_ctx* c)
         CK(aux_swap_stream<double>(c->Q, c->soa, a, c->stream));
     } else {
         StepArgs<float> a = make_args<float>(c, c->pop[0], c->pop[0]);
-        if (pf) a.pf = c->prefetch >= 0 ? c->prefetch : 16384;
+        if (pf) { a.pf = c->prefetch >= 0 ? c->prefetch : 65536; a.pf_strided = 1; }
         CK(aux_swap_stream<float>(c->Q, c->soa, a, c->stream));
     }
     c->launches++;
@@ -488,11 +493,12 @@ lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme
     c->pop_elems = c->soa ? (size_t)c->g.stride * c->Q : (size_t)c->g.n * c->Q;
     c->alloc = g_alloc; c->free_fn = g_free; c->stream = g_stream;
     c->variant = V_DEFAULT;
-    { const char* e = getenv("LBM_PDL"); c->pdl = !(e && e[0] == '0'); }
-    { const char* e = getenv("LBM_PF"); c->prefetch = e ? atoi(e) : -1; }  // -1 = the tuned distances
+    c->pdl = 1;
+    c->prefetch = -1;
     c->block = 128;
     c->n_fluid = c->g.n;
-    lattice_tables(c->Q, c->c, c->opp, c->w);
+    lattice_tables(c->Q, c->c, c->opp, c->w, c->sslot);
+    if (c->soa) for (int k = 0; k < c->Q; ++k) c->sslot[k] = k;
 
     const int narr = c->fam == FAM_2POP ? 2 : 1;
     bool ok = true;
@@ -743,10 +749,10 @@ static int export_planes(lbm_t* c, void* f, const int* cells_dev, int m)
         p.weight = c->w[k];
         const double cu = c->c[kb][0] * c->u_wall[0] + c->c[kb][1] * c->u_wall[1] + c->c[kb][2] * c->u_wall[2];
         p.wterm = -6.0 * c->w[kb] * cu;
-        if (mode == LD_LOCAL) { p.slot_fluid = k; p.slot_wall = k; p.sx = p.sy = p.sz = 0; }
+        if (mode == LD_LOCAL) { p.slot_fluid = c->sslot[k]; p.slot_wall = c->sslot[k]; p.sx = p.sy = p.sz = 0; }
         else {
-            p.slot_fluid = mode == LD_PULL ? k : kb;
-            p.slot_wall = mode == LD_PULL ? kb : k;
+            p.slot_fluid = c->sslot[mode == LD_PULL ? k : kb];
+            p.slot_wall = c->sslot[mode == LD_PULL ? kb : k];
             p.sx = c->c[k][0]; p.sy = c->c[k][1]; p.sz = c->c[k][2];
         }
         char* out = sc + (size_t)(k & 3) * plane;
@@ -800,9 +806,9 @@ int lbm_set_populations(lbm_t* c, const void* f)
         char* in = sc + (size_t)(k & 3) * nb;
         CK(cudaMemcpyAsync(in, (const char*)f + (size_t)k * nb, nb, cudaMemcpyHostToDevice, c->stream));
         if (c->dtype == LBM_F64)
-            CK(aux_insert_plane<double>(c->Q, c->soa, (double*)c->pop[0], c->code, c->g, k, c->w[k], (const double*)in, c->stream));
+            CK(aux_insert_plane<double>(c->Q, c->soa, (double*)c->pop[0], c->code, c->g, c->sslot[k], c->w[k], (const double*)in, c->stream));
         else
-            CK(aux_insert_plane<float>(c->Q, c->soa, (float*)c->pop[0], c->code, c->g, k, c->w[k], (const float*)in, c->stream));
+            CK(aux_insert_plane<float>(c->Q, c->soa, (float*)c->pop[0], c->code, c->g, c->sslot[k], c->w[k], (const float*)in, c->stream));
         c->launches++;
     }
     CK(cudaStreamSynchronize(c->stream));
@@ -1127,6 +1133,8 @@ int lbm_set_variant(lbm_t* c, int variant)
         if (int rc = normalise(c)) return rc;
     }
     c->variant = variant;
+    c->pdl = variant != V_PLAIN;
+    c->prefetch = variant == V_PLAIN ? 0 : -1;
     drop_graph(c);
     return LBM_OK;
 }

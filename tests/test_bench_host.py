@@ -78,3 +78,28 @@ def test_reference_arm_other_ranks_exit_quietly():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "1",
                         "--steps", "2", "--warmup", "1"], capture_output=True, text=True, timeout=600, env=env)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def test_cavity_profile_helpers():
+    """host logic of paper_2010_11751_b200/cavity.py: centre lines and the comparison of two resolutions"""
+    import numpy as np
+    from paper_2010_11751_b200 import cavity
+    n = 8
+    x, y, z = np.meshgrid(np.arange(n), np.arange(n), np.arange(n), indexing="ij")
+    f = 100.0 * x + 10.0 * y + z
+    # even n: the centre lies between the nodes 3 and 4 of the two other axes
+    assert np.allclose(cavity.centre_line(f, 2), 100 * 3.5 + 10 * 3.5 + np.arange(1, n - 1))
+    assert np.allclose(cavity.centre_line(f, 0), 100 * np.arange(1, n - 1) + 10 * 3.5 + 3.5)
+    g = f[:7, :7, :7]
+    assert np.allclose(cavity.centre_line(g, 1), 100 * 3 + 10 * np.arange(1, 6) + 3)
+    pos = cavity.node_positions(n)
+    assert pos[0] == 0.5 / 6 and pos[-1] == 1 - 0.5 / 6 and len(pos) == n - 2
+    # a profile that is linear between the wall values is reproduced exactly at any resolution
+    coarse = {"pos": cavity.node_positions(10).tolist(), "ux_along_z": cavity.node_positions(10).tolist(),
+              "uz_along_x": (0.0 * cavity.node_positions(10)).tolist()}
+    fine = {"pos": cavity.node_positions(18).tolist(), "ux_along_z": cavity.node_positions(18).tolist(),
+            "uz_along_x": (0.0 * cavity.node_positions(18)).tolist()}
+    assert cavity.profile_difference(coarse, fine, "ux_along_z") < 1e-15
+    assert cavity.profile_difference(coarse, fine, "uz_along_x") == 0.0
+    fine["uz_along_x"][3] = 0.25
+    assert abs(cavity.profile_difference(coarse, fine, "uz_along_x") - 0.25) < 1e-15

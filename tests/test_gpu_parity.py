@@ -230,7 +230,7 @@ def test_graph_dropped_when_rates_change(Lbm, oracle):
 
 
 @pytest.mark.parametrize("scheme,dtype", [("AA_SOA", "f64"), ("AA_SOA", "f32"), ("2POP_SOA", "f32"), ("SWAP_SOA", "f64")])
-def test_prefetch_and_dependent_launch_do_not_change_results(Lbm, scheme, dtype, monkeypatch):
+def test_prefetch_and_dependent_launch_do_not_change_results(Lbm, scheme, dtype):
     """the L2 prefetch (on beyond 100 MB of populations) and the programmatic dependent launch are
     pure scheduling: populations after 11 steps are bit for bit those of a run with both off"""
     nx, ny, nz = 112, 96, 130          # 1.4 M cells: 212 MB (fp64) / 106 MB (fp32) per array
@@ -239,9 +239,10 @@ def test_prefetch_and_dependent_launch_do_not_change_results(Lbm, scheme, dtype,
     npdt = np.float32 if dtype == "f32" else np.float64
     cells = np.arange(0, nx * ny * nz, 97, dtype=np.int32)
 
-    def run():
+    def run(variant="default"):
         g = Lbm(nx, ny, nz, lattice=19, collision="TRT", scheme=scheme, omega=1.8, dtype=dtype)
         g.set_flags(fl, (inputs.U_LID, 0.0, 0.0))
+        g.set_variant(variant)
         g.set_graph("off")
         g.init_equilibrium(rho.astype(npdt), u.astype(npdt))
         g.step(11)
@@ -250,9 +251,7 @@ def test_prefetch_and_dependent_launch_do_not_change_results(Lbm, scheme, dtype,
         return f, e
 
     f1, e1 = run()
-    monkeypatch.setenv("LBM_PF", "0")
-    monkeypatch.setenv("LBM_PDL", "0")
-    f0, e0 = run()
+    f0, e0 = run("plain")
     assert np.isfinite(f1).all() and np.array_equal(f0, f1) and e0 == e1
 
 
