@@ -18,7 +18,7 @@ MODELS = {"BGK_W2": 0, "BGK_NW4": 1, "TRT": 2, "RM": 3, "HM": 4, "CM": 5, "CHM":
 SCHEMES = {"2POP_SOA": 0, "2POP_AOS": 1, "SWAP_SOA": 2, "SWAP_AOS": 3, "AA_SOA": 4, "AA_AOS": 5}
 DTYPES = {"f32": 0, "f64": 1}
 NP_DTYPES = {"f32": np.float32, "f64": np.float64}
-VARIANTS = {"default": 0, "generic_push": 1, "generic_pull": 2, "aos_plain": 3, "tma": 4, "no_tma": 5, "plain": 6}
+VARIANTS = {"default": 0, "generic_push": 1, "generic_pull": 2, "aos_plain": 3, "tma": 4, "no_tma": 5, "plain": 6, "aos_march": 7}
 FLUID, WALL, MOVING, GHOST = 0, 1, 2, 3
 
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)

@@ -51,25 +51,65 @@ __global__ void __launch_bounds__(256) classify_kernel(const uint8_t* __restrict
     if ((threadIdx.x & 31) == 0 && i < g.n) grp[i >> 5] = make_uint2((unsigned)__popc(bits), bits);
 }
 
-// pass 2: exclusive prefix sum of grp[].x over the ngrp groups, one block; total[0] = number of edge cells
-__global__ void __launch_bounds__(1024) classify_scan_kernel(uint2* __restrict__ grp, int ngrp, unsigned* __restrict__ total)
+// pass 2: exclusive prefix sum of grp[].x over the ngrp groups, in three launches: per block of 1024
+// groups its sum (sums[b]); one block turns sums[] into exclusive prefixes and leaves the grand total
+// (the number of edge cells) in total[0]; every block then scans its own 1024 entries from its prefix
+__device__ __forceinline__ unsigned block_scan_1024(unsigned v, unsigned* warp_tot)
 {
-    __shared__ unsigned part[1024];
-    const int per = (ngrp + 1023) / 1024;
-    const int lo = min(ngrp, (int)threadIdx.x * per), hi = min(ngrp, lo + per);
-    unsigned s = 0;
-    for (int j = lo; j < hi; ++j) s += grp[j].x;
-    part[threadIdx.x] = s;
+    // inclusive scan over the 1024 threads of the block; warp_tot: 32 unsigned of shared memory
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const unsigned t = __shfl_up_sync(0xffffffffu, v, o);
+        if (lane >= o) v += t;
+    }
+    if (lane == 31) warp_tot[w] = v;
     __syncthreads();
-    for (int o = 1; o < 1024; o <<= 1) {   // inclusive scan of the per-thread sums
-        const unsigned v = threadIdx.x >= (unsigned)o ? part[threadIdx.x - o] : 0u;
+    if (w == 0) {
+        unsigned t = warp_tot[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const unsigned u = __shfl_up_sync(0xffffffffu, t, o);
+            if (lane >= o) t += u;
+        }
+        warp_tot[lane] = t;
+    }
+    __syncthreads();
+    if (w > 0) v += warp_tot[w - 1];
+    return v;
+}
+__global__ void __launch_bounds__(1024) classify_sum_kernel(const uint2* __restrict__ grp, int ngrp, unsigned* __restrict__ sums)
+{
+    __shared__ unsigned wt[32];
+    const int j = blockIdx.x * 1024 + threadIdx.x;
+    const unsigned v = block_scan_1024(j < ngrp ? grp[j].x : 0u, wt);
+    if (threadIdx.x == 1023) sums[blockIdx.x] = v;
+}
+__global__ void __launch_bounds__(1024) classify_scan_sums_kernel(unsigned* __restrict__ sums, int nb, unsigned* __restrict__ total)
+{
+    __shared__ unsigned wt[32];
+    __shared__ unsigned carry;
+    if (threadIdx.x == 0) carry = 0u;
+    __syncthreads();
+    for (int base = 0; base < nb; base += 1024) {
+        const int j = base + threadIdx.x;
+        const unsigned mine = j < nb ? sums[j] : 0u;
+        const unsigned incl = block_scan_1024(mine, wt);
+        const unsigned c = carry;
+        if (j < nb) sums[j] = c + incl - mine;
         __syncthreads();
-        part[threadIdx.x] += v;
+        if (threadIdx.x == 1023) carry = c + incl;
         __syncthreads();
     }
-    unsigned run = part[threadIdx.x] - s;
-    for (int j = lo; j < hi; ++j) { const unsigned cnt = grp[j].x; grp[j].x = run; run += cnt; }
-    if (threadIdx.x == 1023) total[0] = part[1023];
+    if (threadIdx.x == 0) total[0] = carry;
+}
+__global__ void __launch_bounds__(1024) classify_apply_kernel(uint2* __restrict__ grp, int ngrp, const unsigned* __restrict__ sums)
+{
+    __shared__ unsigned wt[32];
+    const int j = blockIdx.x * 1024 + threadIdx.x;
+    const unsigned mine = j < ngrp ? grp[j].x : 0u;
+    const unsigned incl = block_scan_1024(mine, wt);
+    if (j < ngrp) grp[j].x = sums[blockIdx.x] + incl - mine;
 }
 
 // pass 3: the masks of the edge cells, in cell order
@@ -117,12 +157,17 @@ __global__ void __launch_bounds__(256) stream_only_kernel(const StepArgs<T> a)
 
 static inline int blocks_for(int n, int block) { return (n + block - 1) / block; }
 
-cudaError_t aux_classify_codes(int Q, const uint8_t* flags, uint8_t* code, uint2* grp, unsigned* total, const Geo& g, cudaStream_t s)
+// sums: scratch of ceil(ngrp / 1024) unsigned, ngrp = ceil(n / 32)
+cudaError_t aux_classify_codes(int Q, const uint8_t* flags, uint8_t* code, uint2* grp, unsigned* total, unsigned* sums,
+                               const Geo& g, cudaStream_t s)
 {
     if (Q == 19) classify_kernel<19><<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, grp, g);
     else if (Q == 27) classify_kernel<27><<<blocks_for(g.n, 256), 256, 0, s>>>(flags, code, grp, g);
     else return cudaErrorInvalidValue;
-    classify_scan_kernel<<<1, 1024, 0, s>>>(grp, (g.n + 31) / 32, total);
+    const int ngrp = (g.n + 31) / 32, nb = (ngrp + 1023) / 1024;
+    classify_sum_kernel<<<nb, 1024, 0, s>>>(grp, ngrp, sums);
+    classify_scan_sums_kernel<<<1, 1024, 0, s>>>(sums, nb, total);
+    classify_apply_kernel<<<nb, 1024, 0, s>>>(grp, ngrp, sums);
     return cudaGetLastError();
 }
 cudaError_t aux_classify_masks(int Q, const uint8_t* flags, const uint8_t* code, const uint2* grp, unsigned long long* mask,

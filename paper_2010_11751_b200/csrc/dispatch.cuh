@@ -25,6 +25,7 @@ enum Variant {
     V_TMA,           // SoA: loads staged through shared memory by TMA bulk copies (tma_step.cuh)
     V_NO_TMA,        // SoA: never that kernel (one cell per thread, loads into registers, L2 prefetch)
     V_PLAIN,         // as V_NO_TMA, and neither L2 prefetch nor programmatic dependent launch (pure scheduling: same results)
+    V_AOS_MARCH,     // AoS two-population pull: neighbour records in a marching shared-memory tile (aos_march.cuh)
     V_COUNT
 };
 
@@ -35,7 +36,8 @@ cudaError_t launch_step(int kind, bool soa, int block, bool staged, const StepAr
 // defined in aux.cu
 // flags -> code bytes + per-group edge bits and ordinals (+ the number of edge cells in total[0]); then the
 // compact mask array, which the caller allocates from that number
-cudaError_t aux_classify_codes(int Q, const uint8_t* flags, uint8_t* code, uint2* grp, unsigned* total, const Geo& g, cudaStream_t s);
+cudaError_t aux_classify_codes(int Q, const uint8_t* flags, uint8_t* code, uint2* grp, unsigned* total, unsigned* sums,
+                               const Geo& g, cudaStream_t s);
 cudaError_t aux_classify_masks(int Q, const uint8_t* flags, const uint8_t* code, const uint2* grp, unsigned long long* mask,
                                const Geo& g, cudaStream_t s);
 template <class T>

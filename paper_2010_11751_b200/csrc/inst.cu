@@ -3,6 +3,7 @@
 // (see paper_2010_11751_b200/build.py).  fp64 and fp32 (shifted storage, R20).
 #include "dispatch.cuh"
 #include "tma_step.cuh"
+#include "aos_march.cuh"
 
 #ifndef LBM_INST_Q
 #error "compile with -DLBM_INST_Q=19|27 -DLBM_INST_MODEL=0..14"
@@ -13,6 +14,35 @@ namespace lbm {
 template <class T, int Q, int MODEL, bool SOA, int LOAD, int STORE>
 static cudaError_t launch_one(int block, bool staged, const StepArgs<T>& a, cudaStream_t s)
 {
+    // AoS two-population pull, whole lattice, outermost x-layers solid: neighbour records staged in a
+    // marching shared-memory tile (aos_march.cuh)
+    if constexpr (!SOA && LOAD == LD_PULL && STORE == ST_LOCAL) {
+        if (a.march && staged && a.first == 0 && a.end == a.g.n && a.g.nx >= 4) {
+            constexpr int TY = 4, TZ = 32;
+            using G = MarchGeo<T, Q, TY, TZ>;
+            auto kernel = step_kernel_aos_march<T, Q, MODEL, TY, TZ>;
+            static int per_sm = 0, sms = 0;   // per instantiation
+            if (!per_sm) {
+                cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, G::SMEM);
+                if (e != cudaSuccess) return e;
+                int dev = 0;
+                cudaGetDevice(&dev);
+                cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+                e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, TY * TZ, G::SMEM);
+                if (e != cudaSuccess || per_sm < 1) { per_sm = 0; return e != cudaSuccess ? e : cudaErrorLaunchOutOfResources; }
+            }
+            const int tz = (a.g.nz + TZ - 1) / TZ, ty = (a.g.ny + TY - 1) / TY;
+            // x-segments: enough blocks for a few waves; a segment re-reads two layers, so keep it long
+            int nseg = (4 * per_sm * sms + tz * ty - 1) / (tz * ty);
+            const int max_seg = (a.g.nx - 2 + 15) / 16;
+            if (nseg > max_seg) nseg = max_seg;
+            if (nseg < 1) nseg = 1;
+            const int xlen = (a.g.nx - 2 + nseg - 1) / nseg;
+            nseg = (a.g.nx - 2 + xlen - 1) / xlen;
+            kernel<<<dim3(tz, ty, nseg), TY * TZ, G::SMEM, s>>>(a, xlen);
+            return cudaGetLastError();
+        }
+    }
     if constexpr (!SOA && (LOAD == LD_LOCAL || STORE != ST_PUSH)) {
         if (staged && a.first == 0 && a.end == a.g.n) {  // AoS: local accesses through a transposing shared-memory tile (kernels.cuh)
             const int b = block > 128 ? 128 : block;

@@ -58,6 +58,7 @@ struct StepArgs {
     int pf;           // L2 prefetch distance in cells (0 = off), see step_kernel
     int pf_strided;   // one warp in 128/sizeof(T) prefetches, each lane a different line
     int tma;          // host side: run step_kernel_tma (tma_step.cuh) when the launch allows it
+    int march;        // host side: AoS two-population pull may run step_kernel_aos_march (outer x-layers solid)
     Rates<T> rt;
     T wterm[27];  // w_k
     // offsets filled on the host per launch (make_args) so that the kernels add one uniform

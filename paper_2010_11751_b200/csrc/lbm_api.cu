@@ -191,6 +191,7 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
     a.pf = 0;
     a.pf_strided = 0;
     a.tma = 0;
+    a.march = !c->soa && !c->outer_fluid && !c->has_ghost && c->variant == V_AOS_MARCH;
     a.first = c->range_first;
     a.end = c->range_end > 0 ? c->range_end : c->g.n;
     a.rt.omega = (T)c->omega;
@@ -429,8 +430,10 @@ int step_graphed(lbm_ctx* c)
 // synchronises (the number of edge cells sizes the mask array)
 int classify(lbm_ctx* c, const uint8_t* flags_dev)
 {
-    unsigned* total = reinterpret_cast<unsigned*>(c->partial);   // landing spot for one unsigned
-    CK(aux_classify_codes(c->Q, flags_dev, c->code, c->grp, total, c->g, c->stream));
+    // the energy partials (n/256 doubles) double as scratch here: one unsigned for the total, then the
+    // block sums of the prefix scan (n/32768 unsigned)
+    unsigned* total = reinterpret_cast<unsigned*>(c->partial);
+    CK(aux_classify_codes(c->Q, flags_dev, c->code, c->grp, total, total + 4, c->g, c->stream));
     unsigned n_edge = 0;
     CK(cudaMemcpyAsync(&n_edge, total, sizeof n_edge, cudaMemcpyDeviceToHost, c->stream));
     CK(cudaStreamSynchronize(c->stream));
@@ -439,7 +442,7 @@ int classify(lbm_ctx* c, const uint8_t* flags_dev)
     c->mask = (unsigned long long*)dev_alloc(c, sizeof(unsigned long long) * (size_t)(n_edge > 0 ? n_edge : 1));
     if (!c->mask) { set_err("device allocation failed (link masks of %u edge cells)", n_edge); return LBM_E_ALLOC; }
     CK(aux_classify_masks(c->Q, flags_dev, c->code, c->grp, c->mask, c->g, c->stream));
-    c->launches += 3;
+    c->launches += 5;
     CK(cudaStreamSynchronize(c->stream));
     return LBM_OK;
 }

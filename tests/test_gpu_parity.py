@@ -350,3 +350,39 @@ def test_tma_staged_kernels(Lbm, oracle, Q, model, scheme, dtype):
     ref.step(steps)
     assert np.array_equal(g.get_populations(), ref.get_populations())
     g.close(); ref.close()
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("Q,model", [(19, "BGK_W2"), (19, "TRT"), (27, "BGK_W2"), (27, "K")])
+def test_aos_marching_tile_kernel(Lbm, oracle, Q, model, dtype):
+    """the marching-tile kernel of the two-population AoS scheme (aos_march.cuh, variant aos_march; needs
+    the outermost x-layers solid): a cavity with an obstacle inside, ragged in y and z (partial tiles),
+    two x-segments; against the oracle, and bit for bit the default AoS kernels (cooperative gather) and
+    the plain ones (variant aos_plain)"""
+    nx, ny, nz, steps = 36, 23, 70, 7
+    fl = inputs.cavity_flags(nx, ny, nz)
+    fl[10:14, 5:9, 30:40] = inputs.WALL
+    fl[20:22, 12:20, 3:6] = inputs.MOVING
+    uw = (0.02, -0.01, 0.015)
+    rho, u = inputs.seeded_init(nx, ny, nz, 3)
+    npdt = np.float32 if dtype == "f32" else np.float64
+    rho_in, u_in = rho.astype(npdt), u.astype(npdt)
+    o = oracle.Oracle(nx, ny, nz, Q=Q, model=model, omega=1.6)
+    o.set_flags(fl, uw)
+    o.init_equilibrium(rho_in.astype(np.float64), u_in.astype(np.float64))
+    o.step(steps)
+    got = {}
+    for variant in ("aos_march", "default", "aos_plain"):
+        g = Lbm(nx, ny, nz, lattice=Q, collision=model, scheme="2POP_AOS", omega=1.6, dtype=dtype)
+        g.set_flags(fl, uw)
+        g.set_variant(variant)
+        g.init_equilibrium(rho_in, u_in)
+        g.step(steps)
+        if variant == "aos_march":
+            err = pop_error(g, o, fl, Q, oracle, dtype == "f32")
+            assert err <= (TOL64 if dtype == "f64" else TOL32), err
+            assert abs(g.kinetic_energy() - o.kinetic_energy()) <= (1e-12 if dtype == "f64" else 1e-5) * max(1.0, o.kinetic_energy())
+        got[variant] = g.get_populations()
+        g.close()
+    assert np.array_equal(got["aos_march"], got["aos_plain"])
+    assert np.array_equal(got["default"], got["aos_plain"])
