@@ -183,7 +183,10 @@ int lbm_halo_unpack(lbm_t* ctx, int face, const void* buf_dev);
  *   lbm_slab_complete  both merges, lbm_step_finish;
  *   lbm_slab_step(n)   n times post + complete (every slab on its own device and stream).  Several
  *                      slabs on ONE stream must alternate instead: post on all, then complete on all;
- *   lbm_slab_status    LBM_E_STATE if some message never arrived (synchronises). */
+ *   lbm_slab_status    LBM_E_STATE if some message never arrived (synchronises).
+ * A context lives on the CUDA device that was current at lbm_create, and every call on it expects that
+ * device to be current; lbm_slab_link / post / complete / step switch to it themselves, so one host
+ * thread can drive the slabs of several GPUs. */
 int lbm_slab_link(lbm_t* ctx, int face, lbm_t* peer);
 int lbm_slab_export(lbm_t* ctx, void* handle64);
 int lbm_slab_import(lbm_t* ctx, int face, const void* handle64);

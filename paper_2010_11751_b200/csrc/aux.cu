@@ -274,6 +274,14 @@ cudaError_t aux_swap_stream(int Q, bool soa, const StepArgs<T>& a, cudaStream_t 
     cfg.attrs = attr;
     cfg.numAttrs = a.pdl ? 1 : 0;
     cudaError_t e = cudaSuccess;
+    if (!soa) {   // AoS: cooperative exchange of the slot triples (kernels.cuh)
+        const int grid = blocks_for(a.g.n, 128);
+        const size_t smem = (size_t)(128 / 32) * 192 * sizeof(T);
+        if (Q == 19) swap_stream_kernel_aos<T, 19><<<grid, 128, smem, s>>>(a);
+        else if (Q == 27) swap_stream_kernel_aos<T, 27><<<grid, 128, smem, s>>>(a);
+        else return cudaErrorInvalidValue;
+        return cudaGetLastError();
+    }
 #define CALL(QQ, SS)                                                                   \
     {                                                                                  \
         constexpr int G = swap_groups<T, QQ>();                                        \

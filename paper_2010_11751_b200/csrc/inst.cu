@@ -43,6 +43,14 @@ static cudaError_t launch_one(int block, bool staged, const StepArgs<T>& a, cuda
             return cudaGetLastError();
         }
     }
+    // AoS AA odd step, whole lattice: cooperative gather and scatter of the z-triples (kernels.cuh)
+    if constexpr (!SOA && LOAD == LD_AAPULL && STORE == ST_PUSH) {
+        if (staged && a.first == 0 && a.end == a.g.n) {
+            const int b = block > 128 ? 128 : block;
+            step_kernel_aos_odd<T, Q, MODEL><<<(a.g.n + b - 1) / b, b, (size_t)(b / 32) * 96 * sizeof(T), s>>>(a);
+            return cudaGetLastError();
+        }
+    }
     if constexpr (!SOA && (LOAD == LD_LOCAL || STORE != ST_PUSH)) {
         if (staged && a.first == 0 && a.end == a.g.n) {  // AoS: local accesses through a transposing shared-memory tile (kernels.cuh)
             const int b = block > 128 ? 128 : block;

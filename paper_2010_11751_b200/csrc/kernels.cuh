@@ -409,6 +409,75 @@ __device__ __forceinline__ void load_cell_aos_coop(const StepArgs<T>& a, int i, 
     });
 }
 
+// The same for the scatter of the AA odd step (ST_PUSH: pop_k(x + c_k) <- f_out_k): lane l writes slot
+// 1 + dz of record l + dz of the destination z-row.  The lanes park their triples in shared memory and the
+// warp stores the 96 values with three requests of consecutive addresses; the two entries whose source
+// lies in the neighbouring warps (record 0 slot 2, record 31 slot 0) are skipped -- those warps write
+// them, as this one writes the two values that leave its run (lane 0: record -1, lane 31: record 32).
+// Every location is still written exactly once.  Bulk warps only, every lane must call.
+template <class T, int Q>
+__device__ __forceinline__ void store_cell_aos_coop(const StepArgs<T>& a, int i, T* __restrict__ scratch, const T (&f)[Q])
+{
+    using L = Lat<Q>;
+    const int lane = threadIdx.x & 31;
+    T* __restrict__ dst = a.dst;
+    const long long b = (long long)i - lane;
+    const long long A = (long long)a.g.ny * a.g.nz;
+    static_for<9>([&](auto gc) {
+        constexpr int gx = gc / 3 - 1, gy = gc % 3 - 1;
+        constexpr int km = L::dir_of_code((gx + 1) * 9 + (gy + 1) * 3 + 0);
+        constexpr int k0 = L::dir_of_code((gx + 1) * 9 + (gy + 1) * 3 + 1);
+        constexpr int kp = L::dir_of_code((gx + 1) * 9 + (gy + 1) * 3 + 2);
+        const long long D0 = b + (gx * A + gy * (long long)a.g.nz);   // record lane 0 pushes its cz = 0 value into
+        if constexpr (km >= 0 && kp >= 0) {
+            constexpr int gs = L::aos_slot(km);
+            static_for<3>([&](auto dc) {
+                constexpr int dz = dc - 1;
+                constexpr int k = dz < 0 ? km : dz == 0 ? k0 : kp;
+                const int r = lane + dz;
+                if (r >= 0 && r < 32) scratch[3 * r + 1 + dz] = f[k];
+                else dst[(D0 + r) * Q + gs + 1 + dz] = f[k];
+            });
+            __syncwarp();
+            static_for<3>([&](auto jc) {
+                const int e = 32 * jc + lane, rec = e / 3, sl = e - 3 * rec;
+                if (e != 2 && e != 93) dst[(D0 + rec) * Q + gs + sl] = scratch[e];
+            });
+            __syncwarp();
+        } else if constexpr (k0 >= 0) {
+            constexpr int sl = L::aos_slot(k0);
+            dst[(D0 + lane) * Q + sl] = f[k0];
+        }
+    });
+}
+
+// AA odd step in AoS (LD_AAPULL -> ST_PUSH): both sides are neighbour accesses.  Bulk warps gather and
+// scatter cooperatively (above), the others per thread.  Launch with blockDim/32 * 96 * sizeof(T) bytes of
+// dynamic shared memory.
+// register caps as for step_kernel in fp64 (72 / 96 registers); fp32 64 / 85
+template <class T, int Q>
+constexpr int aos_odd_min_blocks() { return sizeof(T) == 8 ? (Q == 19 ? 7 : 5) : (Q == 19 ? 8 : 6); }
+template <class T, int Q, int MODEL>
+__global__ void __launch_bounds__(128, (aos_odd_min_blocks<T, Q>())) step_kernel_aos_odd(const StepArgs<T> a)
+{
+    constexpr bool SHIFT = sizeof(T) == 4;
+    extern __shared__ __align__(16) unsigned char scratch_raw[];
+    T* scratch = reinterpret_cast<T*>(scratch_raw) + (threadIdx.x >> 5) * 96;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const CellState cs = cell_state(a, i, a.g.n);
+    const bool coop = __all_sync(0xffffffffu, cs.active && !cs.masked);
+    T f[Q];
+    if (coop) {
+        load_cell_aos_coop<T, Q, LD_AAPULL>(a, i, scratch, f);
+        collide<Q, MODEL, SHIFT>(f, a.rt);
+        store_cell_aos_coop<T, Q>(a, i, scratch, f);
+    } else if (cs.active) {
+        load_cell<T, Q, false, LD_AAPULL>(a, i, cs.masked, cs.mask, f);
+        collide<Q, MODEL, SHIFT>(f, a.rt);
+        store_cell<T, Q, false, ST_PUSH>(a, i, cs.masked, cs.mask, f);
+    }
+}
+
 // AoS with shared-memory staging.  In the AoS layout pop[N][Q] the Q values of
 // the cells of one block are one contiguous run of blockDim*Q elements, but a warp that reads
 // "slot k of 32 consecutive cells" touches 32 different sectors.  Whatever is LOCAL to the cell
@@ -587,6 +656,89 @@ __device__ __forceinline__ void swap_pairs(const StepArgs<T>& a, int i, const Ce
             }
         });
     }
+}
+
+// Swap pass 2 in AoS for a warp of bulk cells: the pairs of one (cx, cy) group of the half set are the
+// adjacent slot triples of 32 consecutive records on BOTH sides (own records: slots of kbar; the
+// neighbouring z-row: slots of k, shifted by cz), so they move with requests of consecutive addresses
+// through 2 x 96 elements of shared memory (see load_cell_aos_coop / store_cell_aos_coop); the pairs
+// alone in their group are exchanged per thread.  All loads of a group precede its stores, and no two
+// groups touch the same slot.  Every lane must call.
+template <class T, int Q>
+__device__ __forceinline__ void swap_pairs_aos_coop(const StepArgs<T>& a, int i, T* __restrict__ sa, T* __restrict__ sb)
+{
+    using L = Lat<Q>;
+    const int lane = threadIdx.x & 31;
+    T* __restrict__ pop = a.dst;
+    const long long b = (long long)i - lane;
+    const long long A = (long long)a.g.ny * a.g.nz;
+    static_for<9>([&](auto gc) {
+        constexpr int gx = gc / 3 - 1, gy = gc % 3 - 1;
+        constexpr int km = L::dir_of_code((gx + 1) * 9 + (gy + 1) * 3 + 0);
+        constexpr int k0 = L::dir_of_code((gx + 1) * 9 + (gy + 1) * 3 + 1);
+        constexpr int kp = L::dir_of_code((gx + 1) * 9 + (gy + 1) * 3 + 2);
+        const long long D0 = b + (gx * A + gy * (long long)a.g.nz);
+        // a whole group belongs to the half set or to its opposite, except (0, 0, .), where only cz = -1 does
+        if constexpr (km >= 0 && kp >= 0 && k0 >= 0 && km < L::NH && k0 < L::NH && kp < L::NH) {
+            constexpr int gs = L::aos_slot(km);            // neighbour side: slots of k = (gx, gy, dz): gs + 1 + dz
+            constexpr int go = L::aos_slot(L::opp(kp));    // own side: slots of kbar = (-gx, -gy, -dz): go + 1 - dz
+            static_for<3>([&](auto jc) {
+                const int e = 32 * jc + lane, rec = e / 3, sl = e - 3 * rec;
+                sa[e] = pop[(b + rec) * Q + go + sl];
+                sb[e] = pop[(D0 + rec) * Q + gs + sl];
+            });
+            __syncwarp();
+            T va[3], vb[3];
+            static_for<3>([&](auto dc) {
+                constexpr int dz = dc - 1;
+                const int r = lane + dz;
+                va[dc] = sa[3 * lane + 1 - dz];
+                vb[dc] = (r >= 0 && r < 32) ? sb[3 * r + 1 + dz] : pop[(D0 + r) * Q + gs + 1 + dz];
+            });
+            __syncwarp();
+            static_for<3>([&](auto dc) {
+                constexpr int dz = dc - 1;
+                const int r = lane + dz;
+                sa[3 * lane + 1 - dz] = vb[dc];
+                if (r >= 0 && r < 32) sb[3 * r + 1 + dz] = va[dc];
+                else pop[(D0 + r) * Q + gs + 1 + dz] = va[dc];
+            });
+            __syncwarp();
+            static_for<3>([&](auto jc) {
+                const int e = 32 * jc + lane, rec = e / 3, sl = e - 3 * rec;
+                pop[(b + rec) * Q + go + sl] = sa[e];
+                if (e != 2 && e != 93) pop[(D0 + rec) * Q + gs + sl] = sb[e];
+            });
+            __syncwarp();
+        } else {
+            static_for<3>([&](auto dc) {
+                constexpr int dz = dc - 1;
+                constexpr int k = dz < 0 ? km : dz == 0 ? k0 : kp;
+                if constexpr (k >= 0 && k < L::NH) {
+                    constexpr int kb = L::opp(k);
+                    const long long pa = ((long long)i) * Q + L::aos_slot(kb);
+                    const long long pb = ((long long)i + offset<Q, k>(a.g)) * Q + L::aos_slot(k);
+                    const T x = pop[pa], y = pop[pb];
+                    pop[pa] = y;
+                    pop[pb] = x;
+                }
+            });
+        }
+    });
+}
+
+// swap pass 2, AoS: bulk warps exchange cooperatively, the others per thread (one thread group).  Launch
+// with blockDim/32 * 192 * sizeof(T) bytes of dynamic shared memory.
+template <class T, int Q>
+__global__ void __launch_bounds__(128) swap_stream_kernel_aos(const StepArgs<T> a)
+{
+    extern __shared__ __align__(16) unsigned char swap_scratch_raw[];
+    T* sa = reinterpret_cast<T*>(swap_scratch_raw) + (threadIdx.x >> 5) * 192;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const CellState cs = cell_state(a, i, a.g.n);
+    const bool coop = __all_sync(0xffffffffu, cs.active && !cs.masked);
+    if (coop) swap_pairs_aos_coop<T, Q>(a, i, sa, sa + 96);
+    else if (cs.active) swap_pairs<T, Q, false, 1, 0>(a, i, cs);
 }
 
 template <class T, int Q, bool SOA, int G>

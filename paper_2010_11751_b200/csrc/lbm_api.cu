@@ -48,6 +48,7 @@ enum Storage {
 
 struct lbm_ctx {
     int nx, ny, nz, Q, model, scheme, dtype;
+    int device;         // CUDA device that was current at lbm_create: every buffer and the stream live there
     Family fam;
     bool soa;
     double omega, omega_bulk, omega3, omega_hi, trt_magic;
@@ -480,6 +481,7 @@ lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme
     lbm_ctx* c = new (std::nothrow) lbm_ctx();
     if (!c) { set_err("out of host memory"); return nullptr; }
     memset(c, 0, sizeof *c);
+    cudaGetDevice(&c->device);
     c->nx = nx; c->ny = ny; c->nz = nz; c->Q = lattice; c->model = collision; c->scheme = scheme; c->dtype = dtype;
     c->fam = (scheme == LBM_2POP_SOA || scheme == LBM_2POP_AOS) ? FAM_2POP
            : (scheme == LBM_SWAP_SOA || scheme == LBM_SWAP_AOS) ? FAM_SWAP : FAM_AA;
@@ -990,6 +992,14 @@ int lbm_halo_unpack(lbm_t* c, int face, const void* buf)
     return halo_launch(c, false, c->pop[0], p, const_cast<void*>(buf));
 }
 
+// the slab driver may be called for contexts on several devices from one host thread (one process, peer
+// access): it makes the context's device current for the duration of the call
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) { if (cudaGetDevice(&prev) != cudaSuccess) prev = -1; if (prev != dev) cudaSetDevice(dev); else prev = -1; }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
 // ---- the driver: boundary layers -> peer store -> interior -> merge, without the host in between
 // One allocation per context (cudaMalloc, so that it can be shared through CUDA IPC):
 //   recv[face][parity][halo_count] elements | flag[face] (u64) | counter[face] (u32) | status (int)
@@ -1020,8 +1030,20 @@ int lbm_slab_link(lbm_t* c, int face, lbm_t* peer)
         set_err("lbm_slab_link: the neighbouring slab must have the same ny, nz, lattice, scheme and dtype");
         return LBM_E_ARG;
     }
-    if (int rc = slab_alloc(c)) return rc;
-    if (int rc = slab_alloc(peer)) return rc;
+    if (peer->device != c->device) {   // another GPU of this process: the pack kernel stores into its memory
+        int can = 0;
+        if (cudaDeviceCanAccessPeer(&can, c->device, peer->device) != cudaSuccess || !can) {
+            cudaGetLastError();
+            set_err("lbm_slab_link: device %d cannot access the memory of device %d", c->device, peer->device);
+            return LBM_E_ARG;
+        }
+        DeviceGuard g(c->device);
+        const cudaError_t e = cudaDeviceEnablePeerAccess(peer->device, 0);
+        if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled) return cuda_fail("cudaDeviceEnablePeerAccess", e);
+        cudaGetLastError();
+    }
+    { DeviceGuard g(c->device); if (int rc = slab_alloc(c)) return rc; }
+    { DeviceGuard g(peer->device); if (int rc = slab_alloc(peer)) return rc; }
     c->peer_mem[face] = peer->slab_mem;
     return LBM_OK;
 }
@@ -1053,6 +1075,7 @@ int lbm_slab_import(lbm_t* c, int face, const void* handle64)
 int lbm_slab_post(lbm_t* c)
 {
     if (int rc = slab_check(c, "lbm_slab_post")) return rc;
+    DeviceGuard guard(c->device);
     if (int rc = lbm_step_begin(c)) return rc;
     for (int face = 0; face < 2; ++face) {
         if (!c->peer_mem[face]) continue;
@@ -1072,6 +1095,7 @@ int lbm_slab_complete(lbm_t* c)
 {
     if (!c) { set_err("null context"); return LBM_E_ARG; }
     if (c->mid_step != 2) { set_err("lbm_slab_complete without lbm_slab_post"); return LBM_E_STATE; }
+    DeviceGuard guard(c->device);
     for (int face = 0; face < 2; ++face) {
         if (!c->peer_mem[face]) continue;
         HaloArgs p;
