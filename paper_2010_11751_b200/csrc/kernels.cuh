@@ -756,8 +756,8 @@ swap_stream_kernel(const StepArgs<T> a)
             // one warp in 32 with a line per lane in fp32 (pass 2 in fp32 ran at 77 % of the copy rate with
             // 18 prefetch instructions in every thread)
             const long long reach = (long long)a.g.ny * a.g.nz + a.g.nz + 1;
-            if (a.pf > 0 && !a.pf_strided) {
-                if ((long long)i + a.pf + reach < a.g.n) {
+            if constexpr (sizeof(T) == 8) {
+                if (a.pf > 0 && (long long)i + a.pf + reach < a.g.n) {
                     using L = Lat<Q>;
                     static_for<L::NH>([&](auto kc) {
                         constexpr int k = kc, kb = L::opp(k);
