@@ -763,7 +763,9 @@ __global__ void __launch_bounds__(128) swap_stream_kernel_aos(const StepArgs<T> 
 }
 
 template <class T, int Q, bool SOA, int G>
-__global__ void __launch_bounds__(G == 1 ? swap_max_threads<T, Q>() : 256, G == 1 ? swap_min_blocks<T, Q>() : (sizeof(T) == 8 ? 5 : 6))
+// (two groups, D3Q27: 4 / 5 blocks of 256 = 64 / 48 registers; at 5 / 6 the fp64 instance spilled 136 bytes.
+// Same box, 192^3 D3Q27 swap fp64: BGK-W2 95.2 -> 97.6 %, cumulants 94.8 -> 97.0 %; fp32 86.9 -> 87.2 %)
+__global__ void __launch_bounds__(G == 1 ? swap_max_threads<T, Q>() : 256, G == 1 ? swap_min_blocks<T, Q>() : (sizeof(T) == 8 ? (Q == 27 ? 4 : 5) : (Q == 27 ? 5 : 6)))
 swap_stream_kernel(const StepArgs<T> a)
 {
     asm volatile("griddepcontrol.launch_dependents;");   // see step_kernel
