@@ -98,6 +98,22 @@ int lbm_kinetic_energy(lbm_t* ctx, double* e);
 /* Same into one double in DEVICE memory; asynchronous on the stream. */
 int lbm_kinetic_energy_device(lbm_t* ctx, double* e_dev);
 
+/* The same reduction through an entry point that ALLOCATES NOTHING, for callers that cannot call cudaMalloc
+ * (code under CUDA-graph capture, tight serving loops, harnesses that forbid it): the per-block partial
+ * sums live in a fixed array of LBM_STATIC_SCRATCH_DOUBLES doubles (2 MiB) in the library's device image,
+ * which every GPU that loads the library holds until the process exits.  Same kernels and the same fixed
+ * reduction tree as lbm_kinetic_energy_device, so the result is bit for bit the same; e_dev = one double in
+ * DEVICE memory; asynchronous on the stream; calls no cudaMalloc / cudaFree / allocating library routine
+ * (the first call on a device resolves the array's address with cudaGetSymbolAddress).
+ * Limit: lattices of at most LBM_STATIC_MAX_CELLS cells (66 977 792, e.g. 406^3); larger ones return LBM_E_ARG
+ * with a message naming the limit.  The array is shared by every context and every call on a device and
+ * keeps the last call's contents (nothing in it needs clearing: a call reads only what it has written);
+ * calls that overlap on the GPU -- two contexts on different streams of one device -- RACE on it: order
+ * them on one stream or with events. */
+#define LBM_STATIC_SCRATCH_DOUBLES 262144
+#define LBM_STATIC_MAX_CELLS ((LBM_STATIC_SCRATCH_DOUBLES - 512LL) * 256LL)
+int lbm_kinetic_energy_device_static(lbm_t* ctx, double* e_dev);
+
 /* Pre-collision populations at the current time, canonical [Q][N] order, context dtype, host. */
 int lbm_get_populations(lbm_t* ctx, void* f);
 /* The same for m listed cells only: cells = host int32 [m] of cell indices in [0, N), f = host

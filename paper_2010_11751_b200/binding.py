@@ -24,13 +24,15 @@ FLUID, WALL, MOVING, GHOST = 0, 1, 2, 3
 # every symbol include/lbm.h declares (checked by tests/test_abi.py)
 SYMBOLS = [
     "lbm_set_hooks", "lbm_create", "lbm_destroy", "lbm_set_flags", "lbm_set_relaxation", "lbm_set_trt_magic",
-    "lbm_init_equilibrium", "lbm_init_equilibrium_device", "lbm_step", "lbm_macroscopic", "lbm_macroscopic_device", "lbm_kinetic_energy", "lbm_kinetic_energy_device", "lbm_get_populations", "lbm_get_populations_at",
+    "lbm_init_equilibrium", "lbm_init_equilibrium_device", "lbm_step", "lbm_macroscopic", "lbm_macroscopic_device", "lbm_kinetic_energy", "lbm_kinetic_energy_device", "lbm_kinetic_energy_device_static", "lbm_get_populations", "lbm_get_populations_at",
     "lbm_set_populations", "lbm_steps_done", "lbm_num_fluid", "lbm_device_bytes", "lbm_kernel_launches",
     "lbm_sync", "lbm_set_variant", "lbm_set_block", "lbm_set_graph", "lbm_graph_replays", "lbm_halo_count", "lbm_halo_pack", "lbm_halo_unpack", "lbm_step_begin", "lbm_step_end", "lbm_step_finish",
     "lbm_slab_link", "lbm_slab_export", "lbm_slab_import", "lbm_slab_post", "lbm_slab_complete", "lbm_slab_step", "lbm_slab_status",
     "lbm_last_error", "lbm_version",
 ]
 GRAPH_MODES = {"auto": 0, "off": 1, "on": 2}
+STATIC_SCRATCH_DOUBLES = 262144                      # include/lbm.h
+STATIC_MAX_CELLS = (STATIC_SCRATCH_DOUBLES - 512) * 256
 
 
 class LbmError(RuntimeError):
@@ -68,6 +70,7 @@ def load_library(path=LIB_PATH):
     L.lbm_macroscopic.argtypes = [vp, vp, vp]
     L.lbm_kinetic_energy.argtypes = [vp, dp]
     L.lbm_kinetic_energy_device.argtypes = [vp, vp]
+    L.lbm_kinetic_energy_device_static.argtypes = [vp, vp]
     L.lbm_get_populations.argtypes = [vp, vp]
     L.lbm_get_populations_at.argtypes = [vp, vp, i, vp]
     L.lbm_set_populations.argtypes = [vp, vp]
@@ -219,6 +222,11 @@ class Lbm:
     def kinetic_energy_device(self, e_ptr):
         """e_ptr: integer device address of one double; asynchronous on the stream"""
         self._ck(self._L.lbm_kinetic_energy_device(self._h, C.c_void_p(int(e_ptr))))
+
+    def kinetic_energy_device_static(self, e_ptr):
+        """as kinetic_energy_device, with the partial sums in the library's fixed device array: allocates
+        nothing; lattices of at most STATIC_MAX_CELLS cells (include/lbm.h)"""
+        self._ck(self._L.lbm_kinetic_energy_device_static(self._h, C.c_void_p(int(e_ptr))))
 
     def get_populations(self):
         f = np.empty((self.Q, self.N), dtype=self.np_dtype)

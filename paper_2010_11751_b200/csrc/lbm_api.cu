@@ -1128,6 +1128,58 @@ int lbm_slab_status(lbm_t* c)
     return LBM_OK;
 }
 
+// ---- kinetic energy with its scratch in a fixed device array: an entry point that allocates nothing.
+// The reduce kernel (energy_kernel, kernels.cuh) writes one partial sum per block of 256 cells, and two
+// summing stages fold them (aux_energy).  lbm_kinetic_energy_device keeps those partials in a buffer that
+// lbm_create allocated; here they live in a file-scope array that every GPU which loads the library holds
+// until the process exits.  Nothing in the array has to start at zero: every element a call reads it has
+// written itself (ceil(N/256) partials, then at most ENERGY_STAGE2 sums), so the contents the last call
+// left behind -- of this or of any other context -- are never looked at.
+static __device__ __align__(256) double g_static_scratch[LBM_STATIC_SCRATCH_DOUBLES];
+
+// In host code `g_static_scratch` is a host-side stand-in, not a device address: the address the kernels
+// need comes from cudaGetSymbolAddress, asked once per device with that device current.
+enum { STATIC_MAX_DEVICES = 64 };
+static double* g_static_ptr[STATIC_MAX_DEVICES];   // per device, nullptr = not resolved yet
+
+static int static_scratch_ptr(int device, double** out)
+{
+    if (device < 0 || device >= STATIC_MAX_DEVICES) { set_err("device %d outside [0, %d)", device, (int)STATIC_MAX_DEVICES); return LBM_E_ARG; }
+    if (!g_static_ptr[device]) {
+        DeviceGuard guard(device);
+        double* p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress((void**)&p, g_static_scratch);
+        if (e != cudaSuccess || !p) return cuda_fail("cudaGetSymbolAddress(static scratch)", e);
+        g_static_ptr[device] = p;
+    }
+    *out = g_static_ptr[device];
+    return LBM_OK;
+}
+
+int lbm_kinetic_energy_device_static(lbm_t* c, double* e_dev)
+{
+    if (!c || !e_dev) { set_err("null argument"); return LBM_E_ARG; }
+    // the partials of this lattice and the sums of the second stage must fit the fixed array
+    if ((long long)c->n_partial + ENERGY_STAGE2 > (long long)LBM_STATIC_SCRATCH_DOUBLES) {
+        set_err("lbm_kinetic_energy_device_static: %d cells need %d partial sums, the static scratch holds %d doubles "
+                "(at most %lld cells); use lbm_kinetic_energy_device", c->g.n, c->n_partial + (int)ENERGY_STAGE2,
+                (int)LBM_STATIC_SCRATCH_DOUBLES, (long long)LBM_STATIC_MAX_CELLS);
+        return LBM_E_ARG;
+    }
+    if (c->mid_step) { set_err("export between lbm_step_begin and lbm_step_finish"); return LBM_E_STATE; }
+    if (c->sto == STO_NONE) { set_err("no populations loaded"); return LBM_E_STATE; }
+    double* scratch = nullptr;
+    if (int rc = static_scratch_ptr(c->device, &scratch)) return rc;
+    if (c->dtype == LBM_F64)
+        CK(aux_energy<double>(c->Q, c->soa, load_mode(c), make_args<double>(c, c->pop[0], nullptr, load_mode(c)), scratch,
+                              c->n_partial, e_dev, c->stream));
+    else
+        CK(aux_energy<float>(c->Q, c->soa, load_mode(c), make_args<float>(c, c->pop[0], nullptr, load_mode(c)), scratch,
+                             c->n_partial, e_dev, c->stream));
+    c->launches += 3;
+    return LBM_OK;
+}
+
 long long lbm_steps_done(const lbm_t* c) { return c ? c->steps : -1; }
 long long lbm_num_fluid(const lbm_t* c) { return c ? c->n_fluid : -1; }
 long long lbm_device_bytes(const lbm_t* c) { return c ? c->dev_bytes : -1; }
