@@ -43,9 +43,33 @@ static cudaError_t launch_one(int block, bool staged, const StepArgs<T>& a, cuda
             return cudaGetLastError();
         }
     }
+    // AoS two-population pull, whole lattice: blocks cover patches of z-rows so that source rows are shared in L1
+    if constexpr (!SOA && LOAD == LD_PULL && STORE == ST_LOCAL) {
+        if (a.patch && staged && a.first == 0 && a.end == a.g.n) {
+            constexpr int PY = LBM_AOS_PATCH_PY;
+            const dim3 grid = patch_grid(a.g, PY);
+            const size_t smem = ((size_t)32 * PY * Q + (size_t)96 * PY) * sizeof(T);
+            auto kernel = step_kernel_aos_pull_patch<T, Q, MODEL, PY>;
+            if (smem > 48 * 1024) {
+                static bool raised = false;   // per instantiation
+                if (!raised) {
+                    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                    if (e != cudaSuccess) return e;
+                    raised = true;
+                }
+            }
+            kernel<<<grid, 32 * PY, smem, s>>>(a);
+            return cudaGetLastError();
+        }
+    }
     // AoS AA odd step, whole lattice: cooperative gather and scatter of the z-triples (kernels.cuh)
     if constexpr (!SOA && LOAD == LD_AAPULL && STORE == ST_PUSH) {
         if (staged && a.first == 0 && a.end == a.g.n) {
+            static_assert(LBM_AOS_PATCH_PY == 4, "step_kernel_aos_odd has 128 threads");
+            if (a.patch) {
+                step_kernel_aos_odd<T, Q, MODEL, true><<<patch_grid(a.g, LBM_AOS_PATCH_PY), 128, (size_t)4 * 96 * sizeof(T), s>>>(a);
+                return cudaGetLastError();
+            }
             const int b = block > 128 ? 128 : block;
             step_kernel_aos_odd<T, Q, MODEL><<<(a.g.n + b - 1) / b, b, (size_t)(b / 32) * 96 * sizeof(T), s>>>(a);
             return cudaGetLastError();

@@ -59,6 +59,7 @@ struct StepArgs {
     int pf_strided;   // one warp in 128/sizeof(T) prefetches, each lane a different line
     int tma;          // host side: run step_kernel_tma (tma_step.cuh) when the launch allows it
     int march;        // host side: AoS two-population pull may run step_kernel_aos_march (outer x-layers solid)
+    int patch;        // host side: AoS two-population pull runs step_kernel_aos_pull_patch (the default)
     Rates<T> rt;
     T wterm[27];  // w_k
     // offsets filled on the host per launch (make_args) so that the kernels add one uniform
@@ -376,6 +377,22 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
     store_cell<T, Q, SOA, STORE>(a, i, cs.masked, cs.mask, f);
 }
 
+// thread -> cell of the AoS neighbour kernels: a block of 32 * PY threads covers PY z-row segments of 32
+// cells with consecutive y (grid: ceil(nz/32) x ceil(ny/PY) x nx), see step_kernel_aos_pull_patch.  Returns
+// the cell index, or g.n ("no cell": cell_state makes the lane inactive) outside the box.
+#ifndef LBM_AOS_PATCH_PY
+#define LBM_AOS_PATCH_PY 4
+#endif
+template <int PY>
+__device__ __forceinline__ int patch_cell(const Geo& g)
+{
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int z = blockIdx.x * 32 + lane, y = blockIdx.y * PY + w, x = blockIdx.z;
+    if (z >= g.nz || y >= g.ny) return g.n;
+    return (x * g.ny + y) * g.nz + z;
+}
+inline dim3 patch_grid(const Geo& g, int py) { return dim3((g.nz + 31) / 32, (g.ny + py - 1) / py, g.nx); }
+
 // AoS, neighbour side.  A warp that pulls "slot k of 32 consecutive cells" touches 32 different 32-byte
 // sectors and uses 4 or 8 bytes of each; ncu (profiles/r02_aos_*) shows the AoS gathers running at the
 // rate the LSU / L2 deliver such sectors, not at the DRAM rate.  The internal slot order of a record
@@ -478,13 +495,15 @@ __device__ __forceinline__ void store_cell_aos_coop(const StepArgs<T>& a, int i,
 // register caps as for step_kernel in fp64 (72 / 96 registers); fp32 64 / 85
 template <class T, int Q>
 constexpr int aos_odd_min_blocks() { return sizeof(T) == 8 ? (Q == 19 ? 7 : 5) : (Q == 19 ? 8 : 6); }
-template <class T, int Q, int MODEL>
+template <class T, int Q, int MODEL, bool PATCH = false>
 __global__ void __launch_bounds__(128, (aos_odd_min_blocks<T, Q>())) step_kernel_aos_odd(const StepArgs<T> a)
 {
     constexpr bool SHIFT = sizeof(T) == 4;
     extern __shared__ __align__(16) unsigned char scratch_raw[];
     T* scratch = reinterpret_cast<T*>(scratch_raw) + (threadIdx.x >> 5) * 96;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    // PATCH: blocks cover patches of z-rows (patch_cell), so that the source rows of the gather are shared in L1;
+    // in place, every location is read and written by exactly one cell (R4), so any thread -> cell map is valid
+    const int i = PATCH ? patch_cell<LBM_AOS_PATCH_PY>(a.g) : (int)(blockIdx.x * blockDim.x + threadIdx.x);
     const CellState cs = cell_state(a, i, a.g.n);
     const bool coop = __all_sync(0xffffffffu, cs.active && !cs.masked);
     T f[Q];
@@ -586,6 +605,68 @@ __global__ void __launch_bounds__(128) step_kernel_aos(const StepArgs<T> a)
             T* __restrict__ run = a.dst + base * Q;
             for (int e = threadIdx.x; e < nb; e += blockDim.x) run[e] = tile[e];
         }
+    }
+}
+
+// Two-population pull in AoS with a block that covers a PATCH of PY z-row segments (32 cells each) with
+// consecutive y instead of 32 * PY consecutive cells.  The values a destination row (x, y) pulls for the
+// group (gx, gy) come from the source row (x - gx, y - gy), whose records carry all nine groups; with
+// consecutive cells per block every source row is fetched from L2 by up to nine different blocks on
+// different SMs, each using a third of a sector or less (ncu: L2 -> L1 sectors >= L1 sectors, i.e. no L1
+// hit at all, and the kernel runs at the L2's sector rate).  In a patch the rows y .. y+PY-1 of one block
+// want the source rows y-1 .. y+PY of each of the three x-layers, PY + 2 fetches for PY rows instead of
+// 3 PY, and the warps of a block issue their loads within the same few hundred cycles, so the repeats hit
+// in L1 (or merge with the miss in flight).  Everything else as in step_kernel_aos: cooperative gather of
+// the slot triples for bulk warps, masked per-thread path otherwise, results through the transposing
+// tile, one bulk store per warp (32 records are contiguous).  Launch with grid (ceil(nz/32), ceil(ny/PY),
+// nx), 32 * PY threads and (32 PY Q + 96 PY) * sizeof(T) bytes of dynamic shared memory.
+template <class T, int Q, int MODEL, int PY>
+__global__ void __launch_bounds__(32 * PY) step_kernel_aos_pull_patch(const StepArgs<T> a)
+{
+    constexpr bool SHIFT = sizeof(T) == 4;
+    using L = Lat<Q>;
+    extern __shared__ __align__(128) unsigned char tile_raw[];
+    T* tile = reinterpret_cast<T*>(tile_raw);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int z = blockIdx.x * 32 + lane, y = blockIdx.y * PY + w, x = blockIdx.z;
+    const bool inside = z < a.g.nz && y < a.g.ny;
+    const long long il = ((long long)x * a.g.ny + y) * a.g.nz + z;
+    const int i = inside ? (int)il : a.g.n;      // a.g.n: "no cell" for cell_state
+    const CellState cs = cell_state(a, i, a.g.n);
+    T* rec = tile + threadIdx.x * Q;
+    T f[Q];
+    const bool coop = __all_sync(0xffffffffu, cs.active && !cs.masked);
+    if (coop) {
+        T* scratch = tile + (size_t)(32 * PY) * Q + w * 96;
+        load_cell_aos_coop<T, Q, LD_PULL>(a, i, scratch, f);
+    } else if (cs.active) {
+        load_cell<T, Q, false, LD_PULL>(a, i, cs.masked, cs.mask, f);
+    }
+    if (cs.active) {
+        collide<Q, MODEL, SHIFT>(f, a.rt);
+        static_for<Q>([&](auto kc) { constexpr int sl = L::aos_slot(kc); rec[sl] = f[kc]; });
+    } else {
+        static_for<Q>([&](auto kc) { rec[kc] = T(0); });   // solid cells of the written array: zeros (never read)
+    }
+    // the warp's 32 records are one contiguous run of the other array
+    const long long first = il - lane;           // first cell of the warp's run
+    const bool whole = blockIdx.x * 32 + 32 <= a.g.nz && y < a.g.ny;     // warp-uniform
+    const bool bulk = whole && ((first * Q * (long long)sizeof(T)) & 15LL) == 0LL;
+    if (bulk) {
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the records are read by the TMA unit
+        __syncwarp();
+        if (lane == 0) {
+            asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;"
+                         ::"l"(a.dst + first * Q), "r"(aos_smem_addr(tile + (size_t)w * 32 * Q)), "r"((unsigned)(32 * Q * sizeof(T))) : "memory");
+            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+            asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the tile must outlive the copy
+        }
+    } else if (y < a.g.ny) {
+        __syncwarp();
+        const int cells = min(32, a.g.nz - blockIdx.x * 32);             // cells of this warp inside the row
+        const T* __restrict__ from = tile + (size_t)w * 32 * Q;
+        T* __restrict__ run = a.dst + first * Q;
+        for (int e = lane; e < cells * Q; e += 32) run[e] = from[e];
     }
 }
 
@@ -750,6 +831,8 @@ __device__ __forceinline__ void swap_pairs_aos_coop(const StepArgs<T>& a, int i,
 
 // swap pass 2, AoS: bulk warps exchange cooperatively, the others per thread (one thread group).  Launch
 // with blockDim/32 * 192 * sizeof(T) bytes of dynamic shared memory.
+// (blocks over patches of z-rows as in step_kernel_aos_odd were measured here too: no gain, 256^3 D3Q19 fp64
+// 3.557 -> 3.568 ms, D3Q27 cumulants 2.09 -> 2.30 ms; pass 2 keeps consecutive cells per block)
 template <class T, int Q>
 __global__ void __launch_bounds__(128) swap_stream_kernel_aos(const StepArgs<T> a)
 {

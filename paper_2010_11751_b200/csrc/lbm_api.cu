@@ -193,6 +193,7 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
     a.pf_strided = 0;
     a.tma = 0;
     a.march = !c->soa && !c->outer_fluid && !c->has_ghost && c->variant == V_AOS_MARCH;
+    a.patch = !c->soa && c->variant == V_DEFAULT && c->ny <= 65535 && c->nx <= 65535;   // grid.y / grid.z limits
     a.first = c->range_first;
     a.end = c->range_end > 0 ? c->range_end : c->g.n;
     a.rt.omega = (T)c->omega;
