@@ -60,6 +60,7 @@ struct StepArgs {
     int tma;          // host side: run step_kernel_tma (tma_step.cuh) when the launch allows it
     int march;        // host side: AoS two-population pull may run step_kernel_aos_march (outer x-layers solid)
     int patch;        // host side: AoS two-population pull runs step_kernel_aos_pull_patch (the default)
+    int rev;          // the blocks of step_kernel / swap_stream_kernel walk the cells from the top down
     Rates<T> rt;
     T wterm[27];  // w_k
     // offsets filled on the host per launch (make_args) so that the kernels add one uniform
@@ -277,7 +278,7 @@ __device__ __forceinline__ CellState cell_state(const ARGS& a, long long i, int 
 // __launch_bounds__(max_threads, min_blocks) = the register cap 65536 / (max_threads * min_blocks),
 // tuned on B200 per precision and lattice: fp64 D3Q19 128 x 7 (72 registers, 28 warps per SM), fp64
 // D3Q27 128 x 5 (96 registers: 20 warps per SM instead of the 16 that 128 registers allow), fp32 D3Q19 256 x 6 (40), fp32
-// D3Q27 256 x 4 (64).  Launches clamp the block size to max_threads.
+// D3Q27 256 x 5 (48; round 2: 256 x 4 = 64 registers was 1-3 points slower for every model in the AA scheme).  Launches clamp the block size to max_threads.
 #ifndef LBM_MINB_D19
 #define LBM_MINB_D19 7
 #endif
@@ -291,7 +292,7 @@ __device__ __forceinline__ CellState cell_state(const ARGS& a, long long i, int 
 #define LBM_MINB_F 6
 #endif
 #ifndef LBM_MINB_F27
-#define LBM_MINB_F27 4
+#define LBM_MINB_F27 5
 #endif
 template <class T, int Q>
 constexpr int min_blocks() { return sizeof(T) == 4 ? (Q == 19 ? LBM_MINB_F : LBM_MINB_F27) : Q == 19 ? LBM_MINB_D19 : LBM_MINB_D27; }
@@ -317,7 +318,12 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
     // griddepcontrol.wait, i.e. once this grid has completed and its stores are visible.  Without
     // the launch attribute both instructions do nothing.
     asm volatile("griddepcontrol.launch_dependents;");
-    const int i = a.first + blockIdx.x * blockDim.x + threadIdx.x;
+    // a.rev: the blocks walk the cells from the top down.  Successive step kernels alternate the direction
+    // (host: step_kind), so each starts on the ~100 MB of lines its predecessor touched last, which are still
+    // in the 126 MB L2: those reads hit, and in the in-place schemes the lines are overwritten there before
+    // they were ever written back.  Less DRAM traffic than the algorithmic bytes; nothing for the arithmetic.
+    const unsigned blk = a.rev ? gridDim.x - 1u - blockIdx.x : blockIdx.x;
+    const int i = a.first + blk * blockDim.x + threadIdx.x;
     const CellState cs = cell_state(a, i, a.end);
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (!cs.active) {  // solid cells hold no populations
@@ -346,13 +352,13 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
     // cells of each plane (65536 cells ahead).  Measured, same box, prefetch off -> on: AA fp32
     // 88.0 -> 95.2 %, 2-pop fp32 86.7 -> 90.6 %, cumulants AA fp32 82.7 -> 89.1 %, AA fp64 98.9 ->
     // 100.5 %, D3Q27 cumulants AA fp64 92.0 -> 96.2 %, 128^3 AA fp64 94.0 -> 95.9 %.
-    if (a.pf > 0) {
+    if (a.pf != 0) {   // negative: the cells behind, for a kernel that walks downwards
         // keep every prefetched address inside the arrays: a neighbour offset reaches at most one
         // x-layer + one row + one cell beyond the target cell, so stay that far from both ends
         const long long margin = (long long)a.g.ny * a.g.nz + a.g.nz + 1;
         if (!a.pf_strided) {
             const long long t = (long long)i + a.pf;   // 64-bit: N may be close to 2^31
-            if (t >= margin && t + margin < a.g.n && t < a.end) {
+            if (t >= margin && t + margin < a.g.n && t < a.end && t >= a.first) {
                 if constexpr (SOA) {
                     const int ti = (int)t;
                     static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a.lp[kc] + ti)); });
@@ -365,7 +371,7 @@ __global__ void __launch_bounds__(max_threads<T, Q>(), min_blocks<T, Q>()) step_
             constexpr int CPL = 128 / sizeof(T);   // cells per line
             const int lane = threadIdx.x & 31;
             const long long tgt = (long long)(i - lane) + a.pf + (long long)lane * CPL;
-            if ((((i - a.first) >> 5) % CPL) == 0 && tgt >= margin && tgt + CPL + margin < a.g.n && tgt + CPL < a.end) {
+            if ((((i - a.first) >> 5) % CPL) == 0 && tgt >= margin && tgt + CPL + margin < a.g.n && tgt + CPL < a.end && tgt >= a.first) {
                 const int ti = (int)tgt;
                 static_for<Q>([&](auto kc) { asm volatile("prefetch.global.L2 [%0];" ::"l"(a.lp[kc] + ti)); });
             }
@@ -852,7 +858,8 @@ __global__ void __launch_bounds__(G == 1 ? swap_max_threads<T, Q>() : 256, G == 
 swap_stream_kernel(const StepArgs<T> a)
 {
     asm volatile("griddepcontrol.launch_dependents;");   // see step_kernel
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned blk = a.rev ? gridDim.x - 1u - blockIdx.x : blockIdx.x;   // see step_kernel
+    const int i = blk * blockDim.x + threadIdx.x;
     const CellState cs = cell_state<false>(a, i, a.g.n);
     asm volatile("griddepcontrol.wait;" ::: "memory");
     if (!cs.active) return;
@@ -863,7 +870,7 @@ swap_stream_kernel(const StepArgs<T> a)
             // 18 prefetch instructions in every thread)
             const long long reach = (long long)a.g.ny * a.g.nz + a.g.nz + 1;
             if constexpr (sizeof(T) == 8) {
-                if (a.pf > 0 && (long long)i + a.pf + reach < a.g.n) {
+                if (a.pf != 0 && (long long)i + a.pf >= 0 && (long long)i + a.pf + reach < a.g.n) {   // pf < 0: walking downwards
                     using L = Lat<Q>;
                     static_for<L::NH>([&](auto kc) {
                         constexpr int k = kc, kb = L::opp(k);
@@ -873,11 +880,11 @@ swap_stream_kernel(const StepArgs<T> a)
                         }
                     });
                 }
-            } else if (a.pf > 0) {
+            } else if (a.pf != 0) {
                 constexpr int CPL = 128 / sizeof(T);   // cells per line
                 const int lane = threadIdx.x & 31;
                 const long long tgt = (long long)(i - lane) + a.pf + (long long)lane * CPL;
-                if (((i >> 5) % CPL) == 0 && tgt + CPL + reach < a.g.n) {
+                if (((i >> 5) % CPL) == 0 && tgt >= 0 && tgt + CPL + reach < a.g.n) {
                     using L = Lat<Q>;
                     static_for<L::NH>([&](auto kc) {
                         constexpr int k = kc, kb = L::opp(k);

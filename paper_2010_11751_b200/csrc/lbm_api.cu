@@ -57,6 +57,7 @@ struct lbm_ctx {
     size_t elem;        // bytes per population
     size_t pop_elems;   // elements in one population array
     void* pop[2];       // [1] only for FAM_2POP
+    void* pop_first;    // pop[0] as allocated: tells the parity of the two-population pointer exchange
     uint8_t* code;
     uint2* grp;                // per 32 cells: ordinal of the first edge cell, bit set of edge cells (kernels.cuh)
     unsigned long long* mask;  // link masks of the edge cells only, [n_edge]
@@ -192,6 +193,7 @@ StepArgs<T> make_args(const lbm_ctx* c, const void* src, void* dst, int load = L
     a.pf = 0;
     a.pf_strided = 0;
     a.tma = 0;
+    a.rev = 0;
     a.march = !c->soa && !c->outer_fluid && !c->has_ghost && c->variant == V_AOS_MARCH;
     a.patch = !c->soa && c->variant == V_DEFAULT && c->ny <= 65535 && c->nx <= 65535;   // grid.y / grid.z limits
     a.first = c->range_first;
@@ -250,6 +252,10 @@ cudaError_t step_model(const lbm_ctx* c, int kind, const StepArgs<T>& a)
     return cudaErrorInvalidValue;
 }
 
+// the alternating direction pays as soon as the populations do not fit in L2 as a whole (below that every
+// line hits anyway)
+bool beyond_l2_half(const lbm_ctx* c) { return c->pop_elems * c->elem * (c->fam == FAM_2POP ? 2 : 1) > (size_t)60 << 20; }
+
 template <class T>
 cudaError_t step_kind(lbm_ctx* c, int kind, const void* src, void* dst)
 {
@@ -263,6 +269,13 @@ cudaError_t step_kind(lbm_ctx* c, int kind, const void* src, void* dst)
     if (c->soa && beyond_l2 && (kind == SK_EVEN || kind == SK_ODD || kind == SK_PULL)) {
         a.pf_strided = sizeof(T) == 4;
         a.pf = c->prefetch >= 0 ? c->prefetch : (sizeof(T) == 4 ? 65536 : 16384);
+    }
+    // successive step kernels walk the lattice in alternating directions, so that each starts on the lines its
+    // predecessor left in L2 (kernels.cuh): a pure function of the storage state, hence the same inside a
+    // captured graph.  Whole-lattice SoA launches only; variant "plain" walks upwards always.
+    if (c->soa && beyond_l2_half(c) && c->variant != V_PLAIN && c->variant != V_TMA && a.first == 0 && a.end == c->g.n) {
+        a.rev = kind == SK_ODD ? 1 : kind == SK_PULL ? (c->pop[0] != c->pop_first) : 0;
+        if (a.rev) a.pf = -a.pf;
     }
     if (c->soa && c->variant == V_TMA) { a.tma = 1; a.pf = 0; }
     c->launches++;
@@ -299,13 +312,16 @@ int normalise(lbm_ctx* c)
 int swap_pass2(lbm_ctx* c)
 {
     const bool pf = c->soa && c->pop_elems * c->elem > (size_t)100 << 20;  // as in step_kind
+    const bool rev = c->soa && beyond_l2_half(c) && c->variant != V_PLAIN;   // pass 1 walks upwards, pass 2 downwards (step_kind)
     if (c->dtype == LBM_F64) {
         StepArgs<double> a = make_args<double>(c, c->pop[0], c->pop[0]);
         if (pf) a.pf = c->prefetch >= 0 ? c->prefetch : 16384;
+        if (rev) { a.rev = 1; a.pf = -a.pf; }
         CK(aux_swap_stream<double>(c->Q, c->soa, a, c->stream));
     } else {
         StepArgs<float> a = make_args<float>(c, c->pop[0], c->pop[0]);
         if (pf) { a.pf = c->prefetch >= 0 ? c->prefetch : 65536; a.pf_strided = 1; }
+        if (rev) { a.rev = 1; a.pf = -a.pf; }
         CK(aux_swap_stream<float>(c->Q, c->soa, a, c->stream));
     }
     c->launches++;
@@ -510,6 +526,7 @@ lbm_t* lbm_create(int nx, int ny, int nz, int lattice, int collision, int scheme
     bool ok = true;
     for (int a = 0; a < narr && ok; ++a) {
         c->pop[a] = dev_alloc(c, c->pop_elems * c->elem);
+        if (a == 0) c->pop_first = c->pop[0];
         ok = c->pop[a] != nullptr;
         if (ok) ok = cudaMemsetAsync(c->pop[a], 0, c->pop_elems * c->elem, c->stream) == cudaSuccess;
     }
