@@ -136,7 +136,8 @@ int lbm_sync(lbm_t* ctx);
  * the paper's collide-then-push (Table 1); 2 generic_pull: as pull-then-collide with
  * lazily streamed storage (the default); 3 aos_plain: AoS without the shared-memory tile; 4 tma: SoA
  * loads staged through shared memory by TMA bulk copies; 5 no_tma: never that kernel; 6 plain:
- * one cell per thread, no L2 prefetch, no programmatic dependent launch; 7 aos_march: AoS
+ * one cell per thread, no L2 prefetch, no programmatic dependent launch, every kernel walks the cells upwards
+ * (by default successive kernels alternate the direction to reuse what the last one left in L2); 7 aos_march: AoS
  * two-population pull with the neighbour records in a marching shared-memory tile (only when the
  * outermost x-layers hold no fluid or ghost cell; otherwise the default kernels run).  Variants 4
  * and 7 are measured alternatives that lose to the default.  Unknown: LBM_E_ARG. */

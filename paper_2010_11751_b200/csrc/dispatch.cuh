@@ -24,7 +24,8 @@ enum Variant {
     V_AOS_PLAIN,     // AoS without the shared-memory tile (every access a per-thread gather / scatter)
     V_TMA,           // SoA: loads staged through shared memory by TMA bulk copies (tma_step.cuh)
     V_NO_TMA,        // SoA: never that kernel (one cell per thread, loads into registers, L2 prefetch)
-    V_PLAIN,         // as V_NO_TMA, and neither L2 prefetch nor programmatic dependent launch (pure scheduling: same results)
+    V_PLAIN,         // as V_NO_TMA, and neither L2 prefetch nor programmatic dependent launch nor the alternating traversal
+                     // direction (pure scheduling: same results)
     V_AOS_MARCH,     // AoS two-population pull: neighbour records in a marching shared-memory tile (aos_march.cuh)
     V_COUNT
 };
