@@ -272,8 +272,9 @@ cudaError_t step_kind(lbm_ctx* c, int kind, const void* src, void* dst)
     }
     // successive step kernels walk the lattice in alternating directions, so that each starts on the lines its
     // predecessor left in L2 (kernels.cuh): a pure function of the storage state, hence the same inside a
-    // captured graph.  Whole-lattice SoA launches only; variant "plain" walks upwards always.
-    if (c->soa && beyond_l2_half(c) && c->variant != V_PLAIN && c->variant != V_TMA && a.first == 0 && a.end == c->g.n) {
+    // captured graph.  SoA launches, the whole lattice or a range of x-layers (slab steps: the interior
+    // range is nearly the whole slab); variant "plain" walks upwards always.
+    if (c->soa && beyond_l2_half(c) && c->variant != V_PLAIN && c->variant != V_TMA) {
         a.rev = kind == SK_ODD ? 1 : kind == SK_PULL ? (c->pop[0] != c->pop_first) : 0;
         if (a.rev) a.pf = -a.pf;
     }
