@@ -356,3 +356,50 @@ def test_slabs_equal_the_undivided_gpu_run_bitwise(Q, model, scheme, mode):
         energy += e.lbm.kinetic_energy()
         e.close()
     assert abs(energy - e_want) <= 1e-12 * max(1.0, abs(e_want))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("scheme,dtype", [("AA_SOA", "f64"), ("SWAP_SOA", "f64"), ("2POP_SOA", "f32")])
+def test_slabs_beyond_l2_equal_the_undivided_gpu_run_bitwise(scheme, dtype):
+    """slabs large enough (> 60 MB of populations each) for the range launches to alternate their traversal
+    direction and to prefetch: two slabs through the library's peer-store driver reproduce the undivided
+    run bit for bit (sampled cells), odd step count"""
+    from paper_2010_11751_b200 import Lbm
+    NX, NY, NZ, steps = 112, 96, 130, 7
+    omega = 1.8
+    npdt = np.float64 if dtype == "f64" else np.float32
+    fl = inputs.cavity_flags(NX, NY, NZ)
+    uw = (inputs.U_LID, 0.0, 0.0)
+    rho, u = inputs.seeded_init(NX, NY, NZ, 3)
+    rho, u = rho.astype(npdt), u.astype(npdt)
+    g = Lbm(NX, NY, NZ, lattice=19, collision="TRT", scheme=scheme, omega=omega, dtype=dtype)
+    g.set_flags(fl, uw)
+    g.init_equilibrium(rho, u)
+    g.step(steps)
+    cells = np.arange(0, NX * NY * NZ, 53, dtype=np.int64)
+    want = g.get_populations_at(cells.astype(np.int32))
+    e_want = g.kinetic_energy()
+    g.close()
+    engines, ranges = [], []
+    for r in range(2):
+        x0, x1 = slab.slab_range(NX, r, 2)
+        e = slab.GpuSlabEngine(slab.local_flags(fl, x0, x1), uw, lattice=19, collision="TRT", omega=omega, dtype=dtype, scheme=scheme)
+        e.lbm.init_equilibrium(slab.local_field(rho.reshape(NX, NY, NZ), x0, x1),
+                               slab.local_field(u.reshape(3, NX, NY, NZ), x0, x1, axis=1))
+        engines.append(e)
+        ranges.append((x0, x1))
+    slab.link_ring(engines)
+    for _ in range(steps):
+        slab.step_local(engines, mode="peer")
+    energy = 0.0
+    layer = NY * NZ
+    for e, (x0, x1) in zip(engines, ranges):
+        e.lbm.slab_status()
+        mine = cells[(cells >= x0 * layer) & (cells < x1 * layer)]
+        local = (mine - (x0 - 1) * layer).astype(np.int32)      # the slab's context starts one (ghost) layer below x0
+        got = e.lbm.get_populations_at(local)
+        sel = (cells >= x0 * layer) & (cells < x1 * layer)
+        assert np.isfinite(got).all() and np.array_equal(got, want[:, sel])
+        energy += e.lbm.kinetic_energy()
+        e.close()
+    assert abs(energy - e_want) <= (1e-12 if dtype == "f64" else 1e-6) * max(1.0, abs(e_want))
