@@ -1,0 +1,168 @@
+"""Degenerate lattices through the C ABI against the oracle (the edge cases the method has):
+the smallest box the library accepts, 3 x 3 x 3, as a sealed cavity (ONE fluid cell: every link bounces back, the lid
+above it feeds momentum in, Eq 3) and fully periodic (every neighbour is a periodic image and c_k
+applied three times comes back to the cell); a lattice without a single fluid cell; channels one fluid cell thick in
+each of the three directions (rows shorter than a warp, every cell an edge cell); a call for zero steps.  All six
+memory-access schemes, both lattices; tolerances as in tests/test_gpu_parity.py."""
+import numpy as np
+import pytest
+
+from paper_2010_11751_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+
+TOL64 = 1e-12
+TOL32 = 2e-5
+ALL_SCHEMES = ["2POP_SOA", "2POP_AOS", "SWAP_SOA", "SWAP_AOS", "AA_SOA", "AA_AOS"]
+
+
+@pytest.fixture(scope="module")
+def Lbm():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    from paper_2010_11751_b200 import Lbm as cls
+    return cls
+
+
+def _pair(Lbm, oracle, fl, uw, Q, model, scheme, dtype, chunks, omega=1.6, seed=5):
+    nx, ny, nz = fl.shape
+    rho, u = inputs.seeded_init(nx, ny, nz, seed)
+    npdt = np.float32 if dtype == "f32" else np.float64
+    rho_in, u_in = rho.astype(npdt), u.astype(npdt)
+    g = Lbm(nx, ny, nz, lattice=Q, collision=model, scheme=scheme, omega=omega, dtype=dtype)
+    o = oracle.Oracle(nx, ny, nz, Q=Q, model=model, omega=omega)
+    g.set_flags(fl, uw)
+    o.set_flags(fl, uw)
+    g.init_equilibrium(rho_in, u_in)
+    o.init_equilibrium(rho_in.astype(np.float64), u_in.astype(np.float64))
+    for n in chunks:
+        g.step(n)
+    o.step(sum(chunks))
+    assert g.steps_done == sum(chunks)
+    return g, o
+
+
+def _compare(g, o, fl, Q, oracle, dtype):
+    fg = g.get_populations().astype(np.float64)
+    fo = o.get_populations()
+    fluid = fl.reshape(-1) == 0
+    assert np.isfinite(fg).all()
+    assert np.all(fg[:, ~fluid] == 0.0)
+    if fluid.any():
+        d = np.abs(fg - fo)[:, fluid]
+        if dtype == "f64":
+            assert d.max() <= TOL64, d.max()
+        else:
+            _, t, _, _ = oracle.lattice(Q)
+            assert (d / np.maximum(np.abs(fo[:, fluid]), t[:, None])).max() <= TOL32
+    rg, ug = g.macroscopic()
+    ro, uo = o.macroscopic()
+    tol = 1e-12 if dtype == "f64" else 1e-5
+    assert np.abs(rg - ro)[fluid].max(initial=0.0) <= tol and np.abs(ug - uo)[:, fluid].max(initial=0.0) <= tol
+    eg, eo = g.kinetic_energy(), o.kinetic_energy()
+    assert abs(eg - eo) <= (1e-12 if dtype == "f64" else 1e-6) * max(1.0, abs(eo))
+
+
+@pytest.mark.parametrize("Q", [19, 27])
+@pytest.mark.parametrize("scheme", ALL_SCHEMES)
+@pytest.mark.parametrize("kind", ["sealed", "periodic"])
+def test_smallest_box(Lbm, oracle, Q, scheme, kind):
+    """3 x 3 x 3 (smaller extents are refused, tests/test_gpu_parity.py::test_state_errors)"""
+    if kind == "sealed":
+        fl, uw = inputs.cavity_flags(3, 3, 3), (inputs.U_LID, 0.0, 0.0)
+        assert int((fl == 0).sum()) == 1
+    else:
+        fl, uw = inputs.periodic_flags(3, 3, 3), (0.0, 0.0, 0.0)
+    g, o = _pair(Lbm, oracle, fl, uw, Q, "BGK_W2", scheme, "f64", [1, 2, 21])    # odd and even AA parities on the way
+    try:
+        assert g.num_fluid == int((fl == 0).sum())
+        _compare(g, o, fl, Q, oracle, "f64")
+        if kind == "periodic":     # nothing enters or leaves: mass as initialised
+            rho0, _ = inputs.seeded_init(3, 3, 3, 5)
+            assert abs(g.get_populations().sum() - rho0.sum()) <= 1e-12
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("model", ["TRT", "K", "RR"])
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_smallest_box_other_models(Lbm, oracle, model, dtype):
+    for scheme in ("AA_SOA", "SWAP_SOA"):
+        fl = inputs.cavity_flags(3, 3, 3)
+        g, o = _pair(Lbm, oracle, fl, (inputs.U_LID, 0.0, 0.0), 27, model, scheme, dtype, [3, 4])
+        try:
+            _compare(g, o, fl, 27, oracle, dtype)
+        finally:
+            g.close()
+
+
+@pytest.mark.parametrize("scheme", ALL_SCHEMES)
+def test_lattice_without_a_fluid_cell(Lbm, oracle, scheme):
+    """solid cells hold no populations: the steps run, move nothing and the reduce returns 0"""
+    fl = np.full((5, 4, 6), inputs.WALL, dtype=np.uint8)
+    fl[:, :, -1] = inputs.MOVING
+    g, o = _pair(Lbm, oracle, fl, (inputs.U_LID, 0.0, 0.0), 19, "BGK_W2", scheme, "f64", [1, 4])
+    try:
+        assert g.num_fluid == 0
+        assert np.all(g.get_populations() == 0.0)
+        assert g.kinetic_energy() == 0.0 and o.kinetic_energy() == 0.0
+        rho, u = g.macroscopic()
+        assert np.isfinite(rho).all() and np.isfinite(u).all()
+    finally:
+        g.close()
+
+
+def _channel(shape, axis):
+    """periodic box with resting wall on one side and a moving wall on the other side of `axis`, which has 3 cells:
+    one layer of fluid, every fluid cell next to both walls"""
+    fl = inputs.periodic_flags(*shape)
+    assert shape[axis] == 3
+    lo = [slice(None)] * 3
+    hi = [slice(None)] * 3
+    lo[axis], hi[axis] = 0, 2
+    fl[tuple(lo)] = inputs.WALL
+    fl[tuple(hi)] = inputs.MOVING
+    uw = [0.02, -0.01, 0.015]
+    uw[axis] = 0.0                       # the wall moves in its own plane
+    return fl, tuple(uw)
+
+
+@pytest.mark.parametrize("Q", [19, 27])
+@pytest.mark.parametrize("scheme", ALL_SCHEMES)
+@pytest.mark.parametrize("shape,axis", [((9, 3, 40), 1), ((40, 9, 3), 2), ((3, 40, 9), 0)])
+def test_channel_one_cell_thick(Lbm, oracle, Q, scheme, shape, axis):
+    fl, uw = _channel(shape, axis)
+    g, o = _pair(Lbm, oracle, fl, uw, Q, "BGK_W2", scheme, "f64", [5, 20])
+    try:
+        _compare(g, o, fl, Q, oracle, "f64")
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("scheme", ["2POP_SOA", "AA_SOA", "SWAP_AOS"])
+def test_channel_one_cell_thick_fp32_cumulants(Lbm, oracle, scheme):
+    fl, uw = _channel((40, 9, 3), 2)
+    g, o = _pair(Lbm, oracle, fl, uw, 27, "K", scheme, "f32", [5, 20])
+    try:
+        _compare(g, o, fl, 27, oracle, "f32")
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("scheme", ALL_SCHEMES)
+def test_zero_steps_is_a_no_op(Lbm, scheme):
+    fl = inputs.cavity_flags(7, 6, 5)
+    rho, u = inputs.seeded_init(7, 6, 5, 2)
+    g = Lbm(7, 6, 5, scheme=scheme, omega=1.5)
+    try:
+        g.set_flags(fl, (inputs.U_LID, 0.0, 0.0))
+        g.init_equilibrium(rho, u)
+        g.step(3)
+        before = g.get_populations().copy()
+        launches = g.kernel_launches
+        g.step(0)
+        assert g.steps_done == 3
+        assert g.kernel_launches == launches
+        assert np.array_equal(g.get_populations(), before)
+    finally:
+        g.close()
