@@ -166,3 +166,33 @@ def test_zero_steps_is_a_no_op(Lbm, scheme):
         assert np.array_equal(g.get_populations(), before)
     finally:
         g.close()
+
+
+def _pair_variant(Lbm, oracle, fl, uw, Q, scheme, variant, chunks):
+    nx, ny, nz = fl.shape
+    rho, u = inputs.seeded_init(nx, ny, nz, 5)
+    g = Lbm(nx, ny, nz, lattice=Q, collision="BGK_W2", scheme=scheme, omega=1.6)
+    o = oracle.Oracle(nx, ny, nz, Q=Q, model="BGK_W2", omega=1.6)
+    g.set_flags(fl, uw)
+    o.set_flags(fl, uw)
+    g.set_variant(variant)
+    g.init_equilibrium(rho, u)
+    o.init_equilibrium(rho, u)
+    for n in chunks:
+        g.step(n)
+    o.step(sum(chunks))
+    return g, o
+
+
+@pytest.mark.parametrize("variant", ["generic_push", "generic_pull", "aos_plain", "tma", "no_tma", "plain", "aos_march"])
+@pytest.mark.parametrize("scheme", ALL_SCHEMES)
+def test_every_variant_on_the_degenerate_boxes(Lbm, oracle, scheme, variant):
+    """the measured alternatives (include/lbm.h, lbm_set_variant) on lattices smaller than any of their tiles"""
+    cases = [(inputs.periodic_flags(3, 3, 3), (0.0, 0.0, 0.0)), (inputs.cavity_flags(3, 3, 3), (inputs.U_LID, 0.0, 0.0)),
+             _channel((40, 9, 3), 2), _channel((3, 40, 9), 0)]
+    for fl, uw in cases:
+        g, o = _pair_variant(Lbm, oracle, fl, uw, 19, scheme, variant, [1, 18])
+        try:
+            _compare(g, o, fl, 19, oracle, "f64")
+        finally:
+            g.close()
