@@ -196,3 +196,47 @@ def test_every_variant_on_the_degenerate_boxes(Lbm, oracle, scheme, variant):
             _compare(g, o, fl, 19, oracle, "f64")
         finally:
             g.close()
+
+
+@pytest.mark.parametrize("scheme", ALL_SCHEMES)
+@pytest.mark.parametrize("shape", [(4, 4, 32), (3, 5, 33), (5, 3, 31), (3, 4, 128), (3, 3, 257), (7, 4, 96), (3, 9, 5)])
+def test_rows_around_the_warp_and_block_sizes(Lbm, oracle, shape, scheme):
+    """z-rows of exactly one warp, one cell more, one less, one block, two blocks and a cell, three warps, and rows so
+    short that a warp spans six of them: the ragged tails of the thread -> cell maps (linear and AoS patches)"""
+    for kind in ("cavity", "periodic"):
+        fl = inputs.cavity_flags(*shape) if kind == "cavity" else inputs.periodic_flags(*shape)
+        uw = (inputs.U_LID, 0.0, 0.0)
+        g, o = _pair(Lbm, oracle, fl, uw, 19, "BGK_W2", scheme, "f64", [3, 8])
+        try:
+            _compare(g, o, fl, 19, oracle, "f64")
+        finally:
+            g.close()
+
+
+@pytest.mark.parametrize("scheme", ["2POP_SOA", "SWAP_SOA", "AA_SOA", "AA_AOS"])
+@pytest.mark.parametrize("model", ["BGK_W2", "TRT", "HM", "K", "RR", "REG"])
+@pytest.mark.parametrize("omega", [0.05, 1.0, 1.999])
+def test_extreme_relaxation_rates(Lbm, oracle, model, omega, scheme):
+    """omega -> 0 (nearly no collision), omega = 1 (every population replaced by its equilibrium) and omega -> 2 (the
+    zero-viscosity limit, over-relaxation by nearly the full non-equilibrium part), 40 steps of a lid-driven box.
+    (RM and CM are left out: with omega = 0.05 and the other rates at 1 the method itself diverges in these two bases
+    on this box, in the oracle as on the GPU: max |f| 1e9 after 30 steps.)"""
+    fl = inputs.cavity_flags(9, 8, 37)
+    g, o = _pair(Lbm, oracle, fl, (inputs.U_LID, 0.0, 0.0), 27, model, scheme, "f64", [40], omega=omega)
+    try:
+        _compare(g, o, fl, 27, oracle, "f64")
+    finally:
+        g.close()
+
+
+@pytest.mark.parametrize("scheme", ["2POP_SOA", "SWAP_AOS", "AA_SOA"])
+@pytest.mark.parametrize("model", ["BGK_W2", "BGK_NW4", "HM", "CHM", "K", "RR"])
+def test_fast_lid(Lbm, oracle, model, scheme):
+    """a lid at Mach 0.35 (u = 0.2: the velocity-dependent terms of the equilibria and of the moment transforms are
+    no longer small) with components along all three axes in the wall term"""
+    fl = inputs.cavity_flags(8, 9, 35)
+    g, o = _pair(Lbm, oracle, fl, (0.2, -0.05, 0.0), 27, model, scheme, "f64", [30], omega=1.2)
+    try:
+        _compare(g, o, fl, 27, oracle, "f64")
+    finally:
+        g.close()
