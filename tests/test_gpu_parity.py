@@ -266,6 +266,50 @@ def test_every_model_on_every_scheme(Lbm, oracle, Q, scheme, model):
     assert pop_error(g, o, fl, Q, oracle, False) <= TOL64
 
 
+_LONG_ROWS_ORACLE = {}
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("Q", [19, 27])
+@pytest.mark.parametrize("scheme", ALL_SCHEMES)
+@pytest.mark.parametrize("model", ALL_MODELS)
+def test_every_model_on_every_scheme_long_rows(Lbm, oracle, Q, scheme, model, dtype):
+    """the same cross product, in both precisions, on a box whose z-rows (100 cells) hold whole warps of bulk cells:
+    the unmasked access path, the cooperative warp gather / scatter / exchange of the AoS kernels and their patches of
+    four rows run here, next to the masked path of the warps at the walls, the moving block and the periodic seam
+    (on the 7 x 8 x 9 box above every warp has an edge cell).  7 steps in two calls (3 + 4: both AA parities)."""
+    shape, steps = (5, 6, 100), 7
+    key = (Q, model, dtype)
+    fl, uw = box_flags(*shape, "obstacle")
+    rho, u = inputs.seeded_init(*shape, 4)
+    npdt = np.float32 if dtype == "f32" else np.float64
+    rho_in, u_in = rho.astype(npdt), u.astype(npdt)
+    if key not in _LONG_ROWS_ORACLE:          # the oracle's result does not depend on the scheme (PAPER.md:L141)
+        o = oracle.Oracle(*shape, Q=Q, model=model, omega=1.6)
+        o.set_flags(fl, uw)
+        o.init_equilibrium(rho_in.astype(np.float64), u_in.astype(np.float64))
+        o.step(steps)
+        _LONG_ROWS_ORACLE[key] = o.get_populations().copy()
+    fo = _LONG_ROWS_ORACLE[key]
+    g = Lbm(*shape, lattice=Q, collision=model, scheme=scheme, omega=1.6, dtype=dtype)
+    try:
+        g.set_flags(fl, uw)
+        g.init_equilibrium(rho_in, u_in)
+        g.step(3)
+        g.step(4)
+        fg = g.get_populations().astype(np.float64)
+    finally:
+        g.close()
+    fluid = fl.reshape(-1) == 0
+    assert np.isfinite(fg).all() and np.all(fg[:, ~fluid] == 0.0)
+    d = np.abs(fg - fo)[:, fluid]
+    if dtype == "f64":
+        assert d.max() <= TOL64, d.max()
+    else:
+        _, t, _, _ = oracle.lattice(Q)
+        assert (d / np.maximum(np.abs(fo[:, fluid]), t[:, None])).max() <= TOL32
+
+
 @pytest.mark.parametrize("dtype", ["f64", "f32"])
 @pytest.mark.parametrize("Q", [19, 27])
 @pytest.mark.parametrize("model", ["RM", "HM", "CM", "CHM", "K"])
