@@ -229,10 +229,14 @@ def test_graph_dropped_when_rates_change(Lbm, oracle):
     assert pop_error(g, o, fl, 19, oracle, False) <= TOL64
 
 
-@pytest.mark.parametrize("scheme,dtype", [("AA_SOA", "f64"), ("AA_SOA", "f32"), ("2POP_SOA", "f32"), ("SWAP_SOA", "f64")])
-def test_prefetch_and_dependent_launch_do_not_change_results(Lbm, scheme, dtype):
-    """the L2 prefetch (on beyond 100 MB of populations) and the programmatic dependent launch are
-    pure scheduling: populations after 11 steps are bit for bit those of a run with both off"""
+@pytest.mark.parametrize("scheme,dtype,Q,model", [
+    ("AA_SOA", "f64", 19, "TRT"), ("AA_SOA", "f32", 19, "TRT"), ("2POP_SOA", "f32", 19, "TRT"), ("SWAP_SOA", "f64", 19, "TRT"),
+    ("SWAP_SOA", "f32", 19, "TRT"), ("2POP_SOA", "f64", 19, "BGK_W2"), ("AA_SOA", "f32", 27, "K"), ("SWAP_SOA", "f32", 27, "K"),
+    ("2POP_SOA", "f64", 27, "K"), ("SWAP_SOA", "f64", 27, "BGK_W2")])
+def test_prefetch_and_dependent_launch_do_not_change_results(Lbm, scheme, dtype, Q, model):
+    """the L2 prefetch (on beyond 100 MB of populations; per thread in fp64, one strided warp in 32 in fp32, also in
+    swap pass 2), the alternating traversal direction (beyond 60 MB) and the programmatic dependent launch are
+    pure scheduling: populations after 11 steps are bit for bit those of a run with all three off"""
     nx, ny, nz = 112, 96, 130          # 1.4 M cells: 212 MB (fp64) / 106 MB (fp32) per array
     fl = inputs.cavity_flags(nx, ny, nz)
     rho, u = inputs.seeded_init(nx, ny, nz, 9)
@@ -240,7 +244,7 @@ def test_prefetch_and_dependent_launch_do_not_change_results(Lbm, scheme, dtype)
     cells = np.arange(0, nx * ny * nz, 97, dtype=np.int32)
 
     def run(variant="default"):
-        g = Lbm(nx, ny, nz, lattice=19, collision="TRT", scheme=scheme, omega=1.8, dtype=dtype)
+        g = Lbm(nx, ny, nz, lattice=Q, collision=model, scheme=scheme, omega=1.8, dtype=dtype)
         g.set_flags(fl, (inputs.U_LID, 0.0, 0.0))
         g.set_variant(variant)
         g.set_graph("off")
