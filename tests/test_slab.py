@@ -148,7 +148,7 @@ def _flags(kind, NX, NY, NZ):
 
 
 @pytest.mark.gpu
-@pytest.mark.parametrize("Q,dtype", [(19, "f64"), (27, "f64"), (19, "f32")])
+@pytest.mark.parametrize("Q,dtype", [(19, "f64"), (27, "f64"), (19, "f32"), (27, "f32")])
 @pytest.mark.parametrize("kind", ["cavity", "obstacle"])
 @pytest.mark.parametrize("world,mode", [(1, "overlap"), (2, "plain"), (2, "overlap"), (3, "overlap"), (1, "peer"), (2, "peer"), (3, "peer")])
 @pytest.mark.parametrize("scheme", ["2POP_SOA", "AA_SOA", "SWAP_SOA"])
