@@ -276,8 +276,8 @@ def run_gpu(args):
     ms_steps = ev[0].elapsed_time(ev[1])
     ms_macro = ev[1].elapsed_time(ev[2])
     ms_energy = ev[2].elapsed_time(ev[4])
-    assert abs(float(e_d.item()) - energy) == 0.0   # fixed reduction tree: bitwise repeatable
     assert np.isfinite(energy), "simulation blew up"
+    assert abs(float(e_d.item()) - energy) == 0.0   # fixed reduction tree: bitwise repeatable
 
     # ---- end-to-end leg: host buffers in, host buffers out, copies inside the timed region ----
     rho_np, u_np = rho_h.numpy(), u_h.numpy()
